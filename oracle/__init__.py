@@ -1,0 +1,276 @@
+"""ORACLE -- test infrastructure, NOT the product.
+
+ctypes loader for oracle/libzmc_oracle.so (plain single-threaded C++; see
+zmc_oracle.h). Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package; the product
+(paper_1902_07916_b200) never does.
+"""
+import ctypes as C
+from dataclasses import dataclass, field
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+CONST, LINEAR, SIN_SUM, EXP_QUAD = 0, 1, 2, 3
+F64, F32 = 0, 1
+SCOPE_GROUP, SCOPE_POOLED = 0, 1
+BFS, DFS = 0, 1
+
+
+class _Cfg(C.Structure):
+    _fields_ = [
+        ("dim", C.c_int32), ("g", C.c_int32), ("trials", C.c_int32), ("depth", C.c_int32),
+        ("n_samples", C.c_uint64), ("seed", C.c_uint64), ("sigma_multiplier", C.c_double),
+        ("integrand", C.c_int32), ("precision", C.c_int32), ("n_instances", C.c_int32),
+        ("params_per_instance", C.c_int32), ("threshold_scope", C.c_int32), ("traversal", C.c_int32),
+        ("max_groups_per_level", C.c_int64),
+        ("lower", C.POINTER(C.c_double)), ("upper", C.POINTER(C.c_double)), ("params", C.POINTER(C.c_double)),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is not None:
+        return _lib
+    L = C.CDLL(_build.build())
+    u32p, u64p, dp = C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_double)
+    L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
+    L.orc_derive_key.argtypes = [C.c_uint64, C.c_uint32, u32p]
+    L.orc_unit_words.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_uint64, C.c_uint64, u32p]
+    L.orc_cell_geometry.argtypes = [C.c_int, dp, dp, C.c_int, C.c_int, u32p, dp, dp, dp]
+    L.orc_map_f64.argtypes = [C.c_uint32, C.c_double, C.c_double]
+    L.orc_map_f64.restype = C.c_double
+    L.orc_map_f32.argtypes = [C.c_uint32, C.c_double, C.c_double, C.c_double]
+    L.orc_map_f32.restype = C.c_float
+    L.orc_zsin.argtypes = [C.c_float]
+    L.orc_zsin.restype = C.c_float
+    L.orc_zexp.argtypes = [C.c_float, C.POINTER(C.c_int32)]
+    L.orc_zexp.restype = C.c_float
+    L.orc_zexp_value.argtypes = [C.c_float]
+    L.orc_zexp_value.restype = C.c_double
+    L.orc_unit_sum.argtypes = [C.POINTER(_Cfg), C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, dp, dp]
+    L.orc_unit_points.argtypes = [C.POINTER(_Cfg), C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, C.c_uint64, dp, dp]
+    L.orc_cell_stats.argtypes = [dp, C.c_int, C.c_double, C.c_double, C.c_uint64, dp, dp, dp]
+    L.orc_threshold.argtypes = [dp, C.c_int64, C.c_double]
+    L.orc_threshold.restype = C.c_double
+    L.orc_run.argtypes = [C.POINTER(_Cfg), C.c_int]
+    L.orc_run.restype = C.c_void_p
+    L.orc_free.argtypes = [C.c_void_p]
+    L.orc_error.argtypes = [C.c_void_p]
+    L.orc_error.restype = C.c_char_p
+    L.orc_get.argtypes = [C.c_void_p, dp, dp]
+    L.orc_levels.argtypes = [C.c_void_p]
+    L.orc_level_counts.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.orc_total_evals.argtypes = [C.c_void_p]
+    L.orc_total_evals.restype = C.c_uint64
+    L.orc_level_cells.argtypes = [C.c_void_p, C.c_int, u32p, u64p, u32p, dp, dp, dp, C.POINTER(C.c_uint8), dp]
+    L.orc_level_cells.restype = C.c_int64
+    _lib = L
+    return L
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _u32p(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint32))
+
+
+@dataclass
+class Config:
+    """One integration problem (mirrors orc_config)."""
+    dim: int
+    lower: Sequence[float]
+    upper: Sequence[float]
+    g: int
+    n_samples: int
+    trials: int
+    depth: int
+    sigma_multiplier: float
+    seed: int
+    integrand: int
+    precision: int = F64
+    params: Optional[np.ndarray] = None      # [n_instances, params_per_instance]
+    n_instances: int = 1
+    threshold_scope: int = SCOPE_GROUP
+    traversal: int = BFS
+    max_groups_per_level: int = 0
+    _keep: list = field(default_factory=list, repr=False)
+
+    def c(self) -> _Cfg:
+        lo = np.ascontiguousarray(self.lower, dtype=np.float64)
+        up = np.ascontiguousarray(self.upper, dtype=np.float64)
+        if self.params is None:
+            p = np.zeros((self.n_instances, 1), dtype=np.float64)
+            ppi = 0
+        else:
+            p = np.ascontiguousarray(self.params, dtype=np.float64).reshape(self.n_instances, -1)
+            ppi = p.shape[1]
+        self._keep[:] = [lo, up, p]
+        return _Cfg(self.dim, self.g, self.trials, self.depth, self.n_samples, self.seed, self.sigma_multiplier,
+                    self.integrand, self.precision, self.n_instances, ppi, self.threshold_scope, self.traversal,
+                    self.max_groups_per_level, _dp(lo), _dp(up), _dp(p))
+
+
+def philox4x32_10(ctr, key):
+    c = np.asarray(ctr, dtype=np.uint32)
+    k = np.asarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox4x32_10(_u32p(c), _u32p(k), _u32p(out))
+    return out
+
+
+def derive_key(seed, instance=0):
+    out = np.zeros(2, dtype=np.uint32)
+    lib().orc_derive_key(seed, instance, _u32p(out))
+    return out
+
+
+def unit_words(seed, instance, path, level, trial, first_word, n_words):
+    out = np.zeros(n_words, dtype=np.uint32)
+    lib().orc_unit_words(seed, instance, path & (2**64 - 1), path >> 64, level, trial, first_word, n_words, _u32p(out))
+    return out
+
+
+def cell_geometry(dim, lower, upper, g, level, coords):
+    lo_in = np.ascontiguousarray(lower, dtype=np.float64)
+    up_in = np.ascontiguousarray(upper, dtype=np.float64)
+    cc = np.ascontiguousarray(coords, dtype=np.uint32)
+    lo = np.zeros(dim)
+    w = np.zeros(dim)
+    V = C.c_double()
+    lib().orc_cell_geometry(dim, _dp(lo_in), _dp(up_in), g, level, _u32p(cc), _dp(lo), _dp(w), C.byref(V))
+    return lo, w, V.value
+
+
+def map_f64(w, lo, width):
+    return lib().orc_map_f64(int(w), lo, width)
+
+
+def map_f32(w, lo, width, centre=0.0):
+    return np.float32(lib().orc_map_f32(int(w), lo, width, centre))
+
+
+def zsin(a):
+    return np.float32(lib().orc_zsin(float(np.float32(a))))
+
+
+def zexp(e):
+    n = C.c_int32()
+    p = lib().orc_zexp(float(np.float32(e)), C.byref(n))
+    return np.float32(p), n.value
+
+
+def zexp_value(e):
+    return lib().orc_zexp_value(float(np.float32(e)))
+
+
+def path_coords(dim, g, path_digits):
+    """Integer coordinates and path id of the cell reached by child indices `path_digits` (R2)."""
+    k = g ** dim
+    coords = [0] * dim
+    P = 0
+    for j in path_digits:
+        P = P * k + j
+        rem = j
+        for d in range(dim):
+            coords[d] = coords[d] * g + rem % g
+            rem //= g
+    return P, coords
+
+
+def unit_sum(cfg: Config, instance, path, level, coords, trial):
+    cc = np.ascontiguousarray(coords, dtype=np.uint32)
+    S, Sabs = C.c_double(), C.c_double()
+    c = cfg.c()
+    rc = lib().orc_unit_sum(C.byref(c), instance, path & (2**64 - 1), path >> 64, level, _u32p(cc), trial,
+                            C.byref(S), C.byref(Sabs))
+    if rc != 0:
+        raise ValueError("oracle: bad config")
+    return S.value, Sabs.value
+
+
+def unit_points(cfg: Config, instance, path, level, coords, trial, n):
+    cc = np.ascontiguousarray(coords, dtype=np.uint32)
+    x = np.zeros((n, cfg.dim))
+    f = np.zeros(n)
+    c = cfg.c()
+    rc = lib().orc_unit_points(C.byref(c), instance, path & (2**64 - 1), path >> 64, level, _u32p(cc), trial, n, _dp(x), _dp(f))
+    if rc != 0:
+        raise ValueError("oracle: bad config")
+    return x, f
+
+
+def cell_stats(S, volume, prefactor, n_samples):
+    S = np.ascontiguousarray(S, dtype=np.float64)
+    I = np.zeros_like(S)
+    mu, s = C.c_double(), C.c_double()
+    lib().orc_cell_stats(_dp(S), len(S), volume, prefactor, n_samples, _dp(I), C.byref(mu), C.byref(s))
+    return I, mu.value, s.value
+
+
+def threshold(s, m):
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    return lib().orc_threshold(_dp(s), len(s), m)
+
+
+@dataclass
+class Level:
+    n_cells: int
+    n_refined: int
+    n_truncated: int
+    instance: Optional[np.ndarray] = None
+    path: Optional[list] = None
+    mu: Optional[np.ndarray] = None
+    s: Optional[np.ndarray] = None
+    tau: Optional[np.ndarray] = None
+    refined: Optional[np.ndarray] = None
+    S: Optional[np.ndarray] = None
+
+
+@dataclass
+class Result:
+    value: np.ndarray
+    std: np.ndarray
+    levels: list
+    evals: int
+
+
+def run(cfg: Config, keep_cells: bool = False) -> Result:
+    L = lib()
+    c = cfg.c()
+    h = L.orc_run(C.byref(c), 1 if keep_cells else 0)
+    try:
+        err = L.orc_error(h)
+        if err:
+            raise ValueError("oracle: " + err.decode())
+        value = np.zeros(cfg.n_instances)
+        std = np.zeros(cfg.n_instances)
+        L.orc_get(h, _dp(value), _dp(std))
+        levels = []
+        for lev in range(1, L.orc_levels(h) + 1):
+            a, b, t = C.c_int64(), C.c_int64(), C.c_int64()
+            L.orc_level_counts(h, lev, C.byref(a), C.byref(b), C.byref(t))
+            rec = Level(a.value, b.value, t.value)
+            if keep_cells:
+                n = a.value
+                inst = np.zeros(n, dtype=np.uint32)
+                plo = np.zeros(n, dtype=np.uint64)
+                phi = np.zeros(n, dtype=np.uint32)
+                mu, s, tau = np.zeros(n), np.zeros(n), np.zeros(n)
+                ref = np.zeros(n, dtype=np.uint8)
+                S = np.zeros((n, cfg.trials))
+                L.orc_level_cells(h, lev, _u32p(inst), plo.ctypes.data_as(C.POINTER(C.c_uint64)), _u32p(phi),
+                                  _dp(mu), _dp(s), _dp(tau), ref.ctypes.data_as(C.POINTER(C.c_uint8)), _dp(S))
+                rec.instance, rec.mu, rec.s, rec.tau, rec.refined, rec.S = inst, mu, s, tau, ref, S
+                rec.path = [int(phi[i]) << 64 | int(plo[i]) for i in range(n)]
+            levels.append(rec)
+        return Result(value, std, levels, L.orc_total_evals(h))
+    finally:
+        L.orc_free(h)

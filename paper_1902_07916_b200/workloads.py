@@ -1,0 +1,94 @@
+"""Seeded synthetic workloads: the five BASELINE.json configs as plain data.
+
+This module holds NO arithmetic of the method (no RNG stream, no map, no integrand, no
+statistics). It only states problem sizes and generates the input parameter arrays, so it can
+serve the oracle (tests) and the CUDA path alike ("Input recipe").
+
+The paper measures on analytic integrands (Eq. 1 and 2), not on a dataset;
+configs 2, 3 and 5 are those two integrands at BASELINE.json's sizes, configs 1 and 4 are
+BASELINE.json's own.
+"""
+from dataclasses import dataclass, field, replace
+from typing import Optional
+
+import numpy as np
+
+# integrand / precision names shared by the binding and by tests (ids are resolved by each side)
+CONST, LINEAR, SIN_SUM, EXP_QUAD = "const", "linear", "sin_sum", "exp_quad"
+F64, F32 = "f64", "f32"
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    dim: int
+    lower: tuple
+    upper: tuple
+    g: int                      # divisions per axis
+    n_samples: int              # N per cell per trial
+    trials: int                 # T
+    depth: int                  # L
+    sigma_multiplier: float     # m
+    seed: int
+    integrand: str
+    precision: str
+    params: Optional[np.ndarray] = None   # [n_instances, params_per_instance], float64
+    n_instances: int = 1
+    max_groups_per_level: int = 0         # R12 refinement budget (0 = off = paper semantics)
+    note: str = ""
+
+    @property
+    def k(self) -> int:
+        return self.g ** self.dim
+
+    def with_(self, **kw) -> "Workload":
+        return replace(self, **kw)
+
+
+def gaussian_params(dim: int, sigma: float, centre: float = 0.0) -> np.ndarray:
+    """EXP_QUAD parameters [A, a, c_0..c_{D-1}] of the paper's f2 (Eq. 2):
+    A = (2 pi sigma^2)^(-D/2), a = 1/(2 sigma^2)."""
+    A = (2.0 * np.pi * sigma * sigma) ** (-0.5 * dim)
+    a = 1.0 / (2.0 * sigma * sigma)
+    return np.array([[A, a] + [centre] * dim], dtype=np.float64)
+
+
+def batched_params(n: int = 1024, dim: int = 4, seed: int = 4) -> np.ndarray:
+    """Config 4 inputs: a_k log-uniform in [1, 1000], c_k uniform in [0.2, 0.8]^dim, seeded.
+    Values are rounded to float32-representable numbers (the FP32 path would round them anyway;
+    this keeps the closed form and the evaluated function the same function)."""
+    rng = np.random.default_rng(seed)
+    a = 10.0 ** (3.0 * rng.random(n))
+    c = 0.2 + 0.6 * rng.random((n, dim))
+    p = np.empty((n, 2 + dim), dtype=np.float64)
+    p[:, 0] = 1.0
+    p[:, 1] = a.astype(np.float32).astype(np.float64)
+    p[:, 2:] = c.astype(np.float32).astype(np.float64)
+    return p
+
+
+def config1() -> Workload:
+    return Workload("cfg1_sin3d_f64", 3, (0.0,) * 3, (10.0,) * 3, 4, 2000, 5, 2, 1.5, 1, SIN_SUM, F64,
+                    note="BASELINE.json configs[0] (PR1 ref)")
+
+
+def config2(depth: int = 3, budget: int = 0) -> Workload:
+    return Workload("cfg2_sin6d", 6, (0.0,) * 6, (10.0,) * 6, 4, 100000, 5, depth, 1.5, 2, SIN_SUM, F32,
+                    max_groups_per_level=budget, note="BASELINE.json configs[1]; paper f1, Eq. (1)")
+
+
+def config3() -> Workload:
+    return Workload("cfg3_gauss9d", 9, (-1.0,) * 9, (1.0,) * 9, 3, 20000, 5, 4, 1.0, 3, EXP_QUAD, F32,
+                    params=gaussian_params(9, 0.01), note="BASELINE.json configs[2]; paper f2, Eq. (2)")
+
+
+def config4(n_instances: int = 1024) -> Workload:
+    p = batched_params(1024, 4, 4)[:n_instances]
+    return Workload("cfg4_batched4d", 4, (0.0,) * 4, (1.0,) * 4, 6, 4096, 5, 2, 1.5, 4, EXP_QUAD, F32,
+                    params=p, n_instances=n_instances,
+                    note="BASELINE.json configs[3]; sigma_multiplier unspecified there -> 1.5 (reading R11)")
+
+
+def config5(depth: int = 4, budget: int = 0) -> Workload:
+    return Workload("cfg5_sin6d_stress", 6, (0.0,) * 6, (10.0,) * 6, 8, 200000, 10, depth, 1.0, 5, SIN_SUM, F32,
+                    max_groups_per_level=budget, note="BASELINE.json configs[4]")
