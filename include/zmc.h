@@ -1,0 +1,180 @@
+/*
+ * zmc.h -- C ABI of libzmc.so: the B200 (sm_100a) hot path of ZMCintegral
+ * (arXiv:1902.07916): stratified Monte-Carlo over a grid of hyper-rectangular cells
+ * with the heuristic tree search of the paper's section 2.1.
+ *
+ * Citations are "PAPER.md:<line>" (the paper's text) and "DESIGN.md R<n>" (the reading
+ * this build takes where the paper is silent). BASELINE.json names the four core calls
+ * (zmc_create, zmc_set_integrand, zmc_run, zmc_result); the others are what those four
+ * cannot work without (options, workspace, statistics, level dumps for parity tests).
+ *
+ * Conventions for every call
+ *   - return value: ZMC_OK (0) or a negative zmc_status; nothing throws or aborts.
+ *     zmc_last_error(ctx) gives a human-readable reason for the last failure on ctx.
+ *   - every pointer argument marked [host] is caller-owned host memory, read or written
+ *     during the call only (inputs are copied); [device] pointers are CUDA device memory.
+ *   - a context is used from one host thread at a time; distinct contexts are independent.
+ *   - all work is enqueued on the CUDA stream given to zmc_run; only zmc_result,
+ *     zmc_stats and zmc_level_cells synchronise that stream.
+ *   - the library needs a CUDA device; without one zmc_create fails with ZMC_ERR_CUDA.
+ *     There is no CPU fallback of any kind.
+ */
+#ifndef ZMC_H
+#define ZMC_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ZMC_MAX_DIM 16      /* D <= 16 (D <= 12 pre-compiled, 13..16 JIT-compiled) */
+#define ZMC_MAX_DEPTH 15    /* level fits 4 bits of the Philox counter (R3) */
+#define ZMC_MAX_TRIALS 255  /* trial fits 8 bits of the Philox counter (R3) */
+
+typedef enum zmc_status {
+    ZMC_OK = 0,
+    ZMC_ERR_ARG = -1,          /* null pointer, non-finite or empty bounds, counts < 1 ... */
+    ZMC_ERR_RANGE = -2,        /* path > 80 bits, g^depth > 2^32, N*D/4 >= 2^32, trials > 255, depth > 15, dim > 16 */
+    ZMC_ERR_NO_INTEGRAND = -3, /* zmc_run before zmc_set_integrand* */
+    ZMC_ERR_COMPILE = -4,      /* NVRTC failed; the log is in zmc_last_error */
+    ZMC_ERR_CUDA = -5,         /* a CUDA runtime call failed (or no device) */
+    ZMC_ERR_CAPACITY = -6,     /* a level needed more cells than max_cells_per_level; result invalid */
+    ZMC_ERR_NOT_RUN = -7,      /* zmc_result / zmc_stats / zmc_level_cells before zmc_run */
+    ZMC_ERR_STATE = -8         /* option changed after the workspace was fixed, level stats not kept ... */
+} zmc_status;
+
+/* Built-in integrands. params = [n_instances][params_per_instance] doubles.
+ *   ZMC_CONST     f = p[0]                                          (test integrand)
+ *   ZMC_LINEAR    f = p[0] + sum_d p[1+d] x_d                       (test integrand)
+ *   ZMC_SIN_SUM   f = sin(sum_d x_d)            paper f1, Eq. (1); no parameters
+ *   ZMC_EXP_QUAD  f = p[0] * exp(-p[1] * |x - c|^2), c_d = p[2+d]
+ *                 paper f2, Eq. (2), is p[0] = (2 pi sigma^2)^(-D/2), p[1] = 1/(2 sigma^2), c = 0.
+ *                 The prefactor p[0] multiplies each trial estimate, not each sample (R8). */
+enum { ZMC_CONST = 0, ZMC_LINEAR = 1, ZMC_SIN_SUM = 2, ZMC_EXP_QUAD = 3, ZMC_USER = 100 };
+
+/* zmc_set_option keys */
+enum {
+    ZMC_OPT_PRECISION = 1,            /* ZMC_F64 (default) or ZMC_F32: arithmetic of map + integrand; sums are always FP64 */
+    ZMC_OPT_MATH = 2,                 /* ZMC_MATH_EXACT (default): documented IEEE op sequence, bit-comparable with a CPU
+                                         (R8); ZMC_MATH_FAST: MUFU sin/ex2 (FP32 only) */
+    ZMC_OPT_MAX_GROUPS_PER_LEVEL = 3, /* refinement budget B per instance and level, first B flagged cells in path
+                                         order (R12); 0 = off = the paper's semantics (default) */
+    ZMC_OPT_KEEP_LEVEL_STATS = 4,     /* 1: keep every level's per-cell arrays for zmc_level_cells (default 0) */
+    ZMC_OPT_MAX_CELLS_PER_LEVEL = 5,  /* capacity of one level in cells; 0 = auto (default) */
+    ZMC_OPT_GRID_BLOCKS = 6,          /* persistent sampling grid in CTAs; 0 = auto (SM count x resident CTAs) */
+    ZMC_OPT_TARGET_ITEMS = 7          /* a level with fewer (cell,trial) units than this is split into sample chunks
+                                         until it has about this many work items (default 65536) */
+};
+enum { ZMC_F64 = 0, ZMC_F32 = 1 };
+enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };
+
+typedef struct zmc_ctx zmc_ctx; /* opaque; owned by the library between zmc_create and zmc_destroy */
+
+/* The parameters of PAPER.md:87 (section 2.3) in BASELINE.json's order.
+ *   out                [host] receives the context
+ *   dim                D, 1..ZMC_MAX_DIM
+ *   lower, upper       [host] D doubles each: the integration box, upper_d > lower_d, finite
+ *   divisions_per_axis g >= 1: every (sub-)domain is cut into k = g^D equal cells
+ *   samples_per_cell   N >= 1 uniform points per cell per trial
+ *   trials             n1 = T independent repetitions per cell, 1..255
+ *   depth              L = number of levels evaluated; depth 1 = no refinement, 1..15
+ *   sigma_multiplier   m in the threshold tau = mean(s) + m * pstd(s) of one sibling group (R6)
+ *   seed               Philox seed (R3) */
+int zmc_create(zmc_ctx** out, int dim, const double* lower, const double* upper, int divisions_per_axis,
+               uint64_t samples_per_cell, int trials, int depth, double sigma_multiplier, uint64_t seed);
+
+/* Choose a built-in integrand. n_instances >= 1 independent integrals share the geometry and the seed,
+ * each with its own parameters, Philox key, thresholds and (value, std) (R11).
+ * params [host] n_instances*params_per_instance doubles (may be NULL iff params_per_instance == 0). */
+int zmc_set_integrand(zmc_ctx* ctx, int builtin_id, const double* params, int params_per_instance, int n_instances);
+
+/* Choose a user integrand given as CUDA source, JIT-compiled with NVRTC for sm_100a together with the
+ * sampling kernel so that it inlines. cuda_src [host] must define, for the precision in force when
+ * zmc_run is called,
+ *     __device__ float  fn_name(const float*  x, int dim, const float*  p, int np)   (ZMC_F32)
+ *     __device__ double fn_name(const double* x, int dim, const double* p, int np)   (ZMC_F64)
+ * x = the sample point, p = this instance's parameters. Parity with a CPU holds for built-ins only. */
+int zmc_set_integrand_source(zmc_ctx* ctx, const char* cuda_src, const char* fn_name, const double* params,
+                             int params_per_instance, int n_instances);
+
+int zmc_set_option(zmc_ctx* ctx, int key, int64_t value);
+
+/* Device memory the run needs under the options in force. Optional: without zmc_set_workspace the
+ * library allocates with cudaMalloc at the first zmc_run. workspace [device], 256-byte aligned,
+ * caller-owned, must outlive the context or the next zmc_set_workspace. */
+int zmc_workspace_bytes(zmc_ctx* ctx, size_t* bytes);
+int zmc_set_workspace(zmc_ctx* ctx, void* workspace, size_t bytes);
+
+/* Enqueue the whole tree search -- every level's sampling, statistics, threshold, flag and compaction
+ * kernels -- on cuda_stream (a cudaStream_t; NULL = the default stream) and return without
+ * synchronising. No host decision is taken between levels. */
+int zmc_run(zmc_ctx* ctx, void* cuda_stream);
+
+/* Synchronise the run's stream and fetch, per instance, the integral estimate (sum of accepted cell
+ * means) and its standard deviation (sqrt of the sum of accepted cell variances, R7).
+ * value, std [host] n_instances doubles each. Returns ZMC_ERR_CAPACITY if a level overflowed. */
+int zmc_result(zmc_ctx* ctx, double* value, double* std);
+
+typedef struct zmc_level_stats {
+    uint64_t n_groups;     /* sibling groups (= parents) evaluated at this level */
+    uint64_t n_cells;      /* cells evaluated = n_groups * k */
+    uint64_t n_flagged;    /* cells with s > tau (level < L) */
+    uint64_t n_refined;    /* flagged cells passed on to the next level (after budget / capacity) */
+    uint64_t evals;        /* integrand evaluations = n_cells * T * N */
+    float sample_ms;       /* device time of this level's sampling kernel (CUDA events) */
+    float control_ms;      /* device time of this level's statistics/threshold/flag/compaction kernels */
+} zmc_level_stats;
+
+typedef struct zmc_stats_t {
+    int32_t levels;                 /* = depth */
+    int32_t overflow;               /* 1 if some level exceeded max_cells_per_level */
+    uint64_t nonfinite;             /* cells whose mean or std is not finite */
+    uint64_t total_evals;
+    float total_ms;                 /* first kernel to last kernel of the run */
+    int32_t regs_per_thread;        /* sampling kernel */
+    int32_t grid_blocks, block_threads;
+    zmc_level_stats level[ZMC_MAX_DEPTH];
+} zmc_stats_t;
+
+int zmc_stats(zmc_ctx* ctx, zmc_stats_t* out);
+
+/* Per-cell arrays of one level (1-based), in evaluation order = ascending (instance, path); needs
+ * ZMC_OPT_KEEP_LEVEL_STATS. Any [host] pointer may be NULL. capacity = number of cells the arrays can
+ * hold; *n_cells receives the level's cell count (call once with capacity 0 to size them).
+ *   instance[c], path_lo[c], path_hi[c]  cell identity (R2: path P' = P*k + j)
+ *   mu[c], s[c]        mean and population std of the T trial estimates (R5)
+ *   tau[c]             threshold of the cell's sibling group (R6)
+ *   refined[c]         1 if the cell was subdivided
+ *   S[c*T + t]         per-(cell, trial) sum of f over the N samples, FP64 */
+int zmc_level_cells(zmc_ctx* ctx, int level, uint64_t capacity, uint64_t* n_cells, uint32_t* instance,
+                    uint64_t* path_lo, uint32_t* path_hi, double* mu, double* s, double* tau, uint8_t* refined,
+                    double* S);
+
+/* Raw generator access for parity tests (R1, R3): n_words words of the flat stream of unit
+ * (instance, path, level, trial) starting at word index first_word, produced by the device code.
+ * out [host] n_words uint32. */
+int zmc_debug_words(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level, int trial,
+                    uint64_t first_word, uint64_t n_words, uint32_t* out);
+
+/* Sample points and integrand values of the first n samples of one unit, produced by the same device
+ * functions the sampling kernel uses. coords [host] D level-`level` integer cell coordinates.
+ * x [host] n*D doubles (FP32 mode: floats widened; EXP_QUAD in FP32: x - c, R8), f [host] n doubles. */
+int zmc_debug_points(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
+                     const uint32_t* coords, int trial, uint64_t n, double* x, double* f);
+
+/* Issue-rate microbenchmarks of the pipes the path uses (roofline denominator).
+ * which: 0 IMAD.WIDE.U32, 1 LOP3, 2 IMAD.WIDE+LOP3 (Philox round mix), 3 FFMA, 4 FADD, 5 DADD, 6 F2F.F64.F32,
+ *        7 MUFU.SIN, 8 MUFU.EX2, 9 DFMA, 10 Philox4x32-10 calls, 11 I2F.F64.U32, 12 LEA.HI
+ * Returns warp-instructions (which 10: Philox calls x 32 lanes) per SM per clock in *per_sm_clk and the
+ * SM clock seen (clock64 ticks / event time) in *sm_mhz. */
+int zmc_microbench(int which, void* cuda_stream, double* per_sm_clk, double* sm_mhz);
+
+const char* zmc_last_error(const zmc_ctx* ctx);   /* "" if none; valid until the next call on ctx */
+const char* zmc_status_string(int status);
+void zmc_destroy(zmc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ZMC_H */

@@ -1,0 +1,419 @@
+/*
+ * zmc_control.cuh -- the tree-search control kernels that run between two levels' sampling
+ * kernels, entirely on the device (R5-R7, R12):
+ *
+ *   zmc_keys_kernel        derived Philox keys, one call per instance                           (R3)
+ *   zmc_init_kernel        root parents, zeroed results, level-1 plan
+ *   zmc_cell_stats_kernel  per-(cell,trial) partial sums -> S_t -> I_t -> (mu_c, s_c)          (R5)
+ *   zmc_threshold_kernel   per sibling group: tau = mean(s) + m*pstd(s), number of s > tau      (R6)
+ *   zmc_scan_kernel        exclusive scans over groups and instances -> output slots, next plan (R7, R12)
+ *   zmc_scatter_kernel     stable compaction of flagged cells into the next parent list;
+ *                          accepted cells -> per-group (sum mu, sum s^2)                         (R7)
+ *   zmc_accumulate_kernel  per instance: value += sum mu, var += sum s^2                         (R7)
+ *   zmc_finalize_kernel    (value, sqrt(var)) per instance
+ *
+ * Every reduction has a fixed shape (strided partials, then a tree), so repeated runs are
+ * bit-identical. Nothing here is read by the host until zmc_result.
+ */
+#ifndef ZMC_CONTROL_CUH
+#define ZMC_CONTROL_CUH
+#include "zmc_device.cuh"
+
+#define ZMC_CTL_THREADS 256
+#define ZMC_SCAN_THREADS 1024
+
+struct ZmcParents {
+    zu32* inst;
+    zu64* plo;
+    zu32* phi;
+    zu32* coord;   /* [d * stride + G] */
+};
+
+struct ZmcCtlArgs {
+    ZmcLevelInfo* info;     /* array indexed by level, 1..L+1 */
+    zu32 level, L, T, g, D;
+    zu32 n_inst;
+    zu64 k, N;
+    zu32 sample_groups;     /* sample groups per unit = ceil(N / SG) */
+    zu32 target_items, min_chunk_groups;
+    double V;               /* cell volume at this level (R2) */
+    double m;               /* sigma multiplier */
+    zu64 budget;            /* R12; ~0 = off */
+    zu64 cap_par;           /* capacity of a parent list */
+    ZmcParents cur, next;
+    zu64 par_stride;
+    const double* params;
+    zi32 ppi;
+    zi32 prefactor_index;   /* EXP_QUAD: 0 (A = p[0] multiplies each trial estimate); else -1 */
+    const double* partial;
+    double* S;              /* [cell*T + t], or nullptr */
+    double* mu;             /* [cell] */
+    double* s;              /* [cell] */
+    unsigned char* refined; /* [cell], or nullptr */
+    double* tau;            /* [group] */
+    zu64* cnt;              /* [group] flagged cells */
+    zu64* excl;             /* [group] exclusive prefix of cnt over all groups */
+    double* gacc;           /* [group][2] accepted (sum mu, sum s^2) */
+    zu64* gfirst;           /* [instance] first group */
+    zu64* gend;             /* [instance] one past the last group */
+    zu64* out0;             /* [instance] first output slot */
+    double* value;          /* [instance] */
+    double* var;            /* [instance] */
+    zu64* nonfinite;
+    zu32* overflow;
+};
+
+/* plan of one level: how the (cell, trial) units are cut into work items */
+__device__ __forceinline__ void zmc_plan_level(ZmcLevelInfo& li, zu64 n_groups, const ZmcCtlArgs& c) {
+    li.n_groups = n_groups;
+    li.n_cells = n_groups * c.k;
+    const zu64 units = li.n_cells * c.T;
+    zu64 nch = 1;
+    if (units > 0 && units < c.target_items) {
+        nch = (c.target_items + units - 1) / units;
+        zu64 max_ch = c.sample_groups / c.min_chunk_groups;
+        if (max_ch < 1) max_ch = 1;
+        if (nch > max_ch) nch = max_ch;
+    }
+    const zu32 cg = (zu32)((c.sample_groups + nch - 1) / nch);
+    li.chunk_groups = cg;
+    li.n_chunks = (c.sample_groups + cg - 1) / cg;
+    li.n_items = units * li.n_chunks;
+    li.work_ctr = 0;
+    li.n_flagged = 0;
+    li.n_refined = 0;
+}
+
+/* R3: Kd(seed, b) = words 0,1 of Philox(ctr = (b, 0, 0, 0x5A4D4321), key = (seed_lo, seed_hi)) */
+__global__ void zmc_keys_kernel(zu32* keys, zu32 n_inst, zu32 seed_lo, zu32 seed_hi) {
+    for (zu64 b = (zu64)blockIdx.x * blockDim.x + threadIdx.x; b < n_inst; b += (zu64)gridDim.x * blockDim.x) {
+        ZmcKeySchedule ks;
+        ks.init(seed_lo, seed_hi);
+        zu32 w[4];
+        zmc_philox((zu32)b, 0u, 0u, 0x5A4D4321u, ks, w);
+        keys[2 * b] = w[0];
+        keys[2 * b + 1] = w[1];
+    }
+}
+
+/* root parents (path 0, coordinates 0), zeroed results, the level-1 plan */
+__global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    const zu64 tid = (zu64)blockIdx.x * blockDim.x + threadIdx.x;
+    for (zu64 b = tid; b < c.n_inst; b += (zu64)gridDim.x * blockDim.x) {
+        c.cur.inst[b] = (zu32)b;
+        c.cur.plo[b] = 0ull;
+        c.cur.phi[b] = 0u;
+        for (zu32 d = 0; d < c.D; ++d) c.cur.coord[(zu64)d * c.par_stride + b] = 0u;
+        c.value[b] = 0.0;
+        c.var[b] = 0.0;
+    }
+    if (tid == 0) {
+        for (zu32 l = 0; l <= c.L + 1; ++l) {
+            ZmcLevelInfo z;
+            z.n_groups = z.n_cells = z.n_items = z.work_ctr = z.n_flagged = z.n_refined = 0;
+            z.n_chunks = 1; z.chunk_groups = c.sample_groups;
+            if (l != 1) c.info[l] = z;
+        }
+        ZmcLevelInfo li;
+        zmc_plan_level(li, c.n_inst, c);
+        c.info[1] = li;
+        *c.nonfinite = 0ull;
+        *c.overflow = 0u;
+    }
+}
+
+/* R5: S_t = sum of the chunk partials in chunk order ; I_t = ((V*A)*S_t)/(double)N ;
+ * mu = (sum_t I_t)/T ; s = sqrt((sum_t (I_t-mu)^2)/T)  -- two-pass, population form. */
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    const ZmcLevelInfo& li = c.info[c.level];
+    const zu64 n_cells = li.n_cells;
+    const zu32 nch = li.n_chunks;
+    const double dN = (double)c.N, dT = (double)c.T;
+    zu64 bad = 0;
+    for (zu64 cell = (zu64)blockIdx.x * blockDim.x + threadIdx.x; cell < n_cells; cell += (zu64)gridDim.x * blockDim.x) {
+        double A = 1.0;
+        if (c.prefactor_index >= 0) {
+            const zu32 inst = c.cur.inst[cell / c.k];
+            A = c.params[(zu64)inst * (zu64)c.ppi + (zu64)c.prefactor_index];
+        }
+        const double VA = __dmul_rn(c.V, A);
+        const double* p = c.partial + cell * (zu64)c.T * nch;
+        double acc = 0.0;
+        for (zu32 t = 0; t < c.T; ++t) {
+            double S = p[(zu64)t * nch];
+            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)t * nch + ch]);
+            if (c.S) c.S[cell * c.T + t] = S;
+            acc = __dadd_rn(acc, __ddiv_rn(__dmul_rn(VA, S), dN));
+        }
+        const double mu = __ddiv_rn(acc, dT);
+        double q = 0.0;
+        for (zu32 t = 0; t < c.T; ++t) {
+            double S = p[(zu64)t * nch];
+            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)t * nch + ch]);
+            const double d = __dadd_rn(__ddiv_rn(__dmul_rn(VA, S), dN), -mu);
+            q = __dadd_rn(q, __dmul_rn(d, d));
+        }
+        const double sd = __dsqrt_rn(__ddiv_rn(q, dT));
+        c.mu[cell] = mu;
+        c.s[cell] = sd;
+        if (!(fabs(mu) <= 1.7976931348623157e308) || !(fabs(sd) <= 1.7976931348623157e308)) ++bad;
+    }
+    if (bad) atomicAdd(c.nonfinite, bad);
+}
+
+/* fixed-shape block reduction (sum); every thread gets the result */
+__device__ __forceinline__ double zmc_block_sum(double v, double* smem) {
+    const int tid = threadIdx.x;
+    __syncthreads();
+    smem[tid] = v;
+    __syncthreads();
+    for (int off = ZMC_CTL_THREADS / 2; off > 0; off >>= 1) {
+        if (tid < off) smem[tid] = __dadd_rn(smem[tid], smem[tid + off]);
+        __syncthreads();
+    }
+    return smem[0];
+}
+
+__device__ __forceinline__ zu64 zmc_block_sum_u64(zu64 v, zu64* smem) {
+    const int tid = threadIdx.x;
+    __syncthreads();
+    smem[tid] = v;
+    __syncthreads();
+    for (int off = ZMC_CTL_THREADS / 2; off > 0; off >>= 1) {
+        if (tid < off) smem[tid] += smem[tid + off];
+        __syncthreads();
+    }
+    return smem[0];
+}
+
+/* R6: one block per sibling group; tau = mean(s) + m * pstd(s), both moments two-pass, population
+ * form ("the mean and standard deviation of the calculated k standard deviations").
+ * R7: flagged iff level < L and s > tau (strict; NaN compares false). */
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ double smem[ZMC_CTL_THREADS];
+    __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    const zu64 n_groups = c.info[c.level].n_groups;
+    const double dk = (double)c.k;
+    for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
+        const double* s = c.s + G * c.k;
+        double part = 0.0;
+        for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) part = __dadd_rn(part, s[j]);
+        const double mean = __ddiv_rn(zmc_block_sum(part, smem), dk);
+        part = 0.0;
+        for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) {
+            const double d = __dadd_rn(s[j], -mean);
+            part = __dadd_rn(part, __dmul_rn(d, d));
+        }
+        const double pstd = __dsqrt_rn(__ddiv_rn(zmc_block_sum(part, smem), dk));
+        const double tau = __dadd_rn(mean, __dmul_rn(c.m, pstd));
+        zu64 n = 0;
+        if (c.level < c.L)
+            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) n += (s[j] > tau) ? 1ull : 0ull;
+        n = zmc_block_sum_u64(n, smem_u);
+        if (threadIdx.x == 0) { c.tau[G] = tau; c.cnt[G] = n; }
+    }
+}
+
+/* block-wide exclusive scan of one value per thread (ZMC_SCAN_THREADS threads); returns the
+ * exclusive prefix and writes the block total to *total */
+__device__ __forceinline__ zu64 zmc_scan_block_excl(zu64 v, zu64* warp_tot, zu64* total) {
+    const zu32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    zu64 inc = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const zu64 o = __shfl_up_sync(0xFFFFFFFFu, inc, off);
+        if (lane >= (zu32)off) inc += o;
+    }
+    __syncthreads();
+    if (lane == 31u) warp_tot[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        zu64 w = warp_tot[lane];
+        zu64 winc = w;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const zu64 o = __shfl_up_sync(0xFFFFFFFFu, winc, off);
+            if (lane >= (zu32)off) winc += o;
+        }
+        warp_tot[lane] = winc - w;
+        if (lane == 31u) *total = winc;
+    }
+    __syncthreads();
+    return warp_tot[warp] + inc - v;
+}
+
+/* One block. (A) exclusive scan of cnt over groups and the first/last group of every instance
+ * (groups are sorted by instance); (B) per instance: flagged c_b, kept = min(c_b, B) (R12), exclusive
+ * scan -> first output slot; (C) the next level's plan. */
+__global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ zu64 warp_tot[32];
+    __shared__ zu64 total;
+    __shared__ zu64 carry;
+    const zu64 n_groups = c.info[c.level].n_groups;
+    for (zu64 b = threadIdx.x; b < c.n_inst; b += ZMC_SCAN_THREADS) { c.gfirst[b] = 0; c.gend[b] = 0; }
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (zu64 base = 0; base < n_groups; base += ZMC_SCAN_THREADS) {
+        const zu64 G = base + threadIdx.x;
+        const zu64 v = (G < n_groups) ? c.cnt[G] : 0ull;
+        const zu64 ex = zmc_scan_block_excl(v, warp_tot, &total);
+        if (G < n_groups) {
+            c.excl[G] = carry + ex;
+            const zu32 me = c.cur.inst[G];
+            if (G == 0 || c.cur.inst[G - 1] != me) c.gfirst[me] = G;
+            if (G + 1 == n_groups || c.cur.inst[G + 1] != me) c.gend[me] = G + 1;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) carry += total;
+        __syncthreads();
+    }
+    const zu64 total_flagged = carry;
+    __syncthreads();
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (zu64 base = 0; base < c.n_inst; base += ZMC_SCAN_THREADS) {
+        const zu64 b = base + threadIdx.x;
+        zu64 kept = 0;
+        if (b < c.n_inst) {
+            const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
+            if (g1 > g0) {
+                const zu64 cb = c.excl[g1 - 1] + c.cnt[g1 - 1] - c.excl[g0];
+                kept = (cb < c.budget) ? cb : c.budget;
+            }
+        }
+        const zu64 ex = zmc_scan_block_excl(kept, warp_tot, &total);
+        if (b < c.n_inst) c.out0[b] = carry + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        zu64 n_next = carry;
+        if (n_next > c.cap_par) { n_next = c.cap_par; *c.overflow = 1u; }
+        c.info[c.level].n_flagged = total_flagged;
+        c.info[c.level].n_refined = n_next;
+        ZmcLevelInfo li;
+        zmc_plan_level(li, (c.level < c.L) ? n_next : 0ull, c);
+        c.info[c.level + 1] = li;
+    }
+}
+
+/* R7: one block per sibling group. Flagged cells get their rank within the instance (stable, path
+ * order); rank < B (R12) and slot < capacity -> the child record (R2) is written to the next parent
+ * list. Every other cell is accepted: its mu and s^2 go into the group's fixed-shape sums. */
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ double smem[ZMC_CTL_THREADS];
+    __shared__ zu32 warp_cnt[ZMC_CTL_THREADS / 32];
+    __shared__ zu64 run;
+    const zu64 n_groups = c.info[c.level].n_groups;
+    const zu32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
+        const zu32 inst = c.cur.inst[G];
+        const double tau = c.tau[G];
+        const zu64 r0 = c.excl[G] - c.excl[c.gfirst[inst]];   /* flagged cells of this instance in earlier groups */
+        const zu64 slot0 = c.out0[inst];
+        const zu64 plo = c.cur.plo[G];
+        const zu32 phi = c.cur.phi[G];
+        double acc_mu = 0.0, acc_var = 0.0;
+        __syncthreads();
+        if (threadIdx.x == 0) run = 0;
+        __syncthreads();
+        for (zu64 base = 0; base < c.k; base += ZMC_CTL_THREADS) {
+            const zu64 j = base + threadIdx.x;
+            const zu64 cell = G * c.k + j;
+            double sj = 0.0, muj = 0.0;
+            bool flag = false;
+            if (j < c.k) {
+                sj = c.s[cell];
+                muj = c.mu[cell];
+                flag = (c.level < c.L) && (sj > tau);
+            }
+            const zu32 bal = __ballot_sync(0xFFFFFFFFu, flag);
+            if (lane == 0) warp_cnt[warp] = __popc(bal);
+            __syncthreads();
+            zu64 before = run;
+            zu32 tile_total = 0;
+#pragma unroll
+            for (int w = 0; w < ZMC_CTL_THREADS / 32; ++w) {
+                if ((zu32)w < warp) before += warp_cnt[w];
+                tile_total += warp_cnt[w];
+            }
+            const zu64 rank = r0 + before + __popc(bal & ((1u << lane) - 1u));
+            bool kept = false;
+            if (flag && rank < c.budget) {
+                const zu64 slot = slot0 + rank;
+                if (slot < c.cap_par) {
+                    kept = true;
+                    /* R2: P' = P*k + j (80 bits) ; I'_d = I_d*g + j_d, axis 0 least significant */
+                    const zu64 nlo = plo * c.k + j;
+                    const zu64 cy = __umul64hi(plo, c.k) + ((nlo < j) ? 1ull : 0ull);
+                    c.next.inst[slot] = inst;
+                    c.next.plo[slot] = nlo;
+                    c.next.phi[slot] = (zu32)((zu64)phi * c.k + cy);
+                    zu64 rem = j;
+                    for (zu32 d = 0; d < c.D; ++d) {
+                        const zu64 q = rem / c.g;
+                        const zu32 jd = (zu32)(rem - q * c.g);
+                        rem = q;
+                        c.next.coord[(zu64)d * c.par_stride + slot] = c.cur.coord[(zu64)d * c.par_stride + G] * c.g + jd;
+                    }
+                }
+            }
+            if (j < c.k) {
+                if (!kept) { acc_mu = __dadd_rn(acc_mu, muj); acc_var = __dadd_rn(acc_var, __dmul_rn(sj, sj)); }
+                if (c.refined) c.refined[cell] = kept ? 1 : 0;
+            }
+            __syncthreads();
+            if (threadIdx.x == 0) run += tile_total;
+            __syncthreads();
+        }
+        const double gm = zmc_block_sum(acc_mu, smem);
+        const double gv = zmc_block_sum(acc_var, smem);
+        if (threadIdx.x == 0) { c.gacc[2 * G] = gm; c.gacc[2 * G + 1] = gv; }
+    }
+}
+
+/* R7: value_b += sum of accepted mu ; var_b += sum of accepted s^2, one block per instance */
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_accumulate_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ double smem[ZMC_CTL_THREADS];
+    for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
+        const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
+        double am = 0.0, av = 0.0;
+        for (zu64 G = g0 + threadIdx.x; G < g1; G += ZMC_CTL_THREADS) {
+            am = __dadd_rn(am, c.gacc[2 * G]);
+            av = __dadd_rn(av, c.gacc[2 * G + 1]);
+        }
+        const double sm = zmc_block_sum(am, smem);
+        const double sv = zmc_block_sum(av, smem);
+        if (threadIdx.x == 0 && g1 > g0) {
+            c.value[b] = __dadd_rn(c.value[b], sm);
+            c.var[b] = __dadd_rn(c.var[b], sv);
+        }
+    }
+}
+
+/* result[b] = value_b ; result[n_inst + b] = sqrt(var_b) */
+__global__ void zmc_finalize_kernel(const double* value, const double* var, double* result, zu32 n_inst) {
+    for (zu64 b = (zu64)blockIdx.x * blockDim.x + threadIdx.x; b < n_inst; b += (zu64)gridDim.x * blockDim.x) {
+        result[b] = value[b];
+        result[n_inst + b] = __dsqrt_rn(var[b]);
+    }
+}
+
+/* debug: words of one unit's flat stream (R3) */
+__global__ void zmc_words_kernel(const zu32* keys, zu32 inst, zu64 path_lo, zu32 path_hi, zu32 level, zu32 trial,
+                                 zu64 first_word, zu64 n_words, zu32* out) {
+    ZmcKeySchedule ks;
+    ks.init(keys[2 * inst], keys[2 * inst + 1]);
+    ZmcUnitCounter uc;
+    uc.init(path_lo, path_hi, level, trial);
+    for (zu64 i = (zu64)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (zu64)gridDim.x * blockDim.x) {
+        const zu64 idx = first_word + i;
+        zu32 w[4];
+        zmc_philox((zu32)(idx >> 2), uc.c1, uc.c2, uc.c3, ks, w);
+        const zu32 l = (zu32)(idx & 3ull);
+        out[i] = (l == 0) ? w[0] : (l == 1) ? w[1] : (l == 2) ? w[2] : w[3];
+    }
+}
+
+#endif /* ZMC_CONTROL_CUH */

@@ -1,0 +1,522 @@
+/*
+ * zmc_device.cuh -- device code of the fused sampling kernel (sm_100a).
+ *
+ * Philox4x32-10 -> word -> point -> integrand -> FP64 sum, all in registers: no sample is ever
+ * written to memory ("produce the random number at the time when using it").
+ * One warp processes one work item = (cell, trial, sample chunk); a persistent grid pulls items
+ * from a device counter whose bound was written by the previous level's control kernels, so the
+ * host enqueues all levels up front.
+ *
+ * This file is self-contained (no #include) because it is compiled twice: ahead of time by nvcc
+ * for the built-in integrands (zmc_inst_*.cu) and at run time by NVRTC for user integrands and
+ * for dimensions without a pre-compiled instance (zmc_lib.cu embeds this text).
+ * It shares nothing with oracle/: the operation sequences below restate DESIGN.md R1-R8.
+ *
+ * Compile with --fmad=false: every fused multiply-add here is written explicitly.
+ */
+#ifndef ZMC_DEVICE_CUH
+#define ZMC_DEVICE_CUH
+
+typedef unsigned int zu32;
+typedef unsigned long long zu64;
+typedef int zi32;
+
+#define ZMC_DEV_MAX_DIM 16
+#ifndef ZMC_BLOCK_THREADS
+#define ZMC_BLOCK_THREADS 128
+#endif
+#ifndef ZMC_MIN_BLOCKS
+#define ZMC_MIN_BLOCKS 4
+#endif
+
+/* integrand ids / precision / math mode: values mirror include/zmc.h (checked by static_assert in zmc_lib.cu) */
+#define ZMC_ID_CONST 0
+#define ZMC_ID_LINEAR 1
+#define ZMC_ID_SIN_SUM 2
+#define ZMC_ID_EXP_QUAD 3
+#define ZMC_ID_USER 100
+#define ZMC_PREC_F64 0
+#define ZMC_PREC_F32 1
+#define ZMC_MODE_EXACT 0
+#define ZMC_MODE_FAST 1
+
+/* One per level (index 1..L) in device memory. Written by the previous level's control kernels
+ * (level 1: by the init kernel); read by this level's kernels. */
+struct ZmcLevelInfo {
+    zu64 n_groups;      /* parents = sibling groups at this level */
+    zu64 n_cells;       /* n_groups * k */
+    zu64 n_items;       /* n_cells * T * n_chunks work items */
+    zu64 work_ctr;      /* the persistent grid's item counter */
+    zu64 n_flagged;     /* cells with s > tau */
+    zu64 n_refined;     /* flagged cells passed on (after budget and capacity) */
+    zu32 n_chunks;      /* sample chunks per (cell, trial) unit */
+    zu32 chunk_groups;  /* sample groups per chunk */
+};
+
+struct ZmcSampleArgs {
+    const zu32* par_inst;    /* [G] instance of each parent */
+    const zu64* par_plo;     /* [G] parent path, low 64 bits */
+    const zu32* par_phi;     /* [G] parent path, bits 64..79 */
+    const zu32* par_coord;   /* [d * par_stride + G] parent integer coordinates */
+    zu64 par_stride;
+    ZmcLevelInfo* info;      /* this level's */
+    double* partial;         /* [item] FP64 partial sums, item = (cell*T + trial)*n_chunks + chunk */
+    const zu32* keys;        /* [instance][2] derived Philox keys (R3) */
+    const double* params;    /* [instance][ppi] */
+    const float* params_f32; /* the same rounded to FP32 (user integrands) */
+    zi32 ppi;
+    zu32 g, T, level;
+    zu64 k;
+    zu64 N;
+    double lower[ZMC_DEV_MAX_DIM];
+    double width[ZMC_DEV_MAX_DIM];   /* cell width at this level, (upper-lower)/g^level (R2) */
+};
+
+/* ------------------------------------------------------------------ R1: Philox4x32-10 */
+/* Salmon, Moraes, Dror, Shaw, "Parallel random numbers: as easy as 1, 2, 3" (SC'11).
+ * round: (hi0,lo0) = M0*c0 ; (hi1,lo1) = M1*c2 ; c <- (hi1^c1^k0, lo1, hi0^c3^k1, lo0) ; k += W.
+ * Each round is 2 IMAD.WIDE.U32 + 2 LOP3 in SASS; the ten key values are loop-invariant. */
+#define ZMC_PHILOX_M0 0xD2511F53u
+#define ZMC_PHILOX_M1 0xCD9E8D57u
+#define ZMC_PHILOX_W0 0x9E3779B9u
+#define ZMC_PHILOX_W1 0xBB67AE85u
+
+struct ZmcKeySchedule {
+    zu32 k0[10], k1[10];
+    __device__ __forceinline__ void init(zu32 key0, zu32 key1) {
+#pragma unroll
+        for (int r = 0; r < 10; ++r) { k0[r] = key0 + (zu32)r * ZMC_PHILOX_W0; k1[r] = key1 + (zu32)r * ZMC_PHILOX_W1; }
+    }
+};
+
+__device__ __forceinline__ void zmc_philox(zu32 c0, zu32 c1, zu32 c2, zu32 c3, const ZmcKeySchedule& ks, zu32* out) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const zu64 p0 = (zu64)c0 * (zu64)ZMC_PHILOX_M0;
+        const zu64 p1 = (zu64)c2 * (zu64)ZMC_PHILOX_M1;
+        const zu32 n0 = (zu32)(p1 >> 32) ^ c1 ^ ks.k0[r];
+        const zu32 n2 = (zu32)(p0 >> 32) ^ c3 ^ ks.k1[r];
+        c1 = (zu32)p1;
+        c3 = (zu32)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* R3: counter of call q of unit (path P, level l, trial t): (q, t | l<<8 | P[79:64]<<16, P[31:0], P[63:32]) */
+struct ZmcUnitCounter {
+    zu32 c1, c2, c3;
+    __device__ __forceinline__ void init(zu64 path_lo, zu32 path_hi, zu32 level, zu32 trial) {
+        c1 = trial | (level << 8) | ((path_hi & 0xFFFFu) << 16);
+        c2 = (zu32)path_lo;
+        c3 = (zu32)(path_lo >> 32);
+    }
+};
+
+/* ------------------------------------------------------------------ R8: FP32 elementary functions (exact mode) */
+/* zsin: k = rint(a/pi) by the magic-number add, two-constant Cody-Waite reduction, odd degree-9
+ * polynomial on [-pi/2, pi/2], sign (-1)^k taken from the low bit of the magic sum. */
+__device__ __forceinline__ float zmc_zsin(float a) {
+    const float INV_PI = __uint_as_float(0x3ea2f983u);
+    const float MAGIC = __uint_as_float(0x4b400000u);
+    const float NPI_A = __uint_as_float(0xc0490000u);   /* -3.140625 */
+    const float NPI_B = __uint_as_float(0xba7daa22u);   /* -fl(pi - 3.140625) */
+    const float C3 = __uint_as_float(0xbe2aaaa6u), C5 = __uint_as_float(0x3c08876au);
+    const float C7 = __uint_as_float(0xb94fb7f7u), C9 = __uint_as_float(0x362ede75u);
+    const float t = __fmaf_rn(a, INV_PI, MAGIC);
+    const float kf = __fadd_rn(t, -MAGIC);
+    float r = __fmaf_rn(kf, NPI_A, a);
+    r = __fmaf_rn(kf, NPI_B, r);
+    const float s = __fmul_rn(r, r);
+    float p = __fmaf_rn(C9, s, C7);
+    p = __fmaf_rn(p, s, C5);
+    p = __fmaf_rn(p, s, C3);
+    const float rs = __fmul_rn(r, s);
+    const float v = __fmaf_rn(rs, p, r);
+    return __uint_as_float(__float_as_uint(v) ^ (__float_as_uint(t) << 31));
+}
+
+/* zexp: n = rint(e*log2 e) by the magic-number add, two-constant reduction r = e - n ln2, degree-6
+ * polynomial p ~ exp(r); exp(e) = p * 2^n is assembled as an FP64 number by adding n to the
+ * exponent field of (double)p, so the FP64 exponent range is available (R9: the 9-D Gaussian's
+ * samples at level 1 lie far below FP32's range). |e| > 708 and NaN take the slow branch. */
+__device__ __forceinline__ double zmc_zexp_value(float e) {
+    if (!(fabsf(e) <= 708.0f)) {
+        if (e < 0.0f) return 0.0;
+        if (e > 0.0f) return __longlong_as_double(0x7FF0000000000000ll);
+        return __longlong_as_double(0x7FF8000000000000ll);
+    }
+    const float LOG2E = __uint_as_float(0x3fb8aa3bu);
+    const float MAGIC = __uint_as_float(0x4b400000u);
+    const float NLN2_HI = __uint_as_float(0xbf317200u);
+    const float NLN2_LO = __uint_as_float(0xb5bfbe8eu);
+    const float E2 = __uint_as_float(0x3efffffeu), E3 = __uint_as_float(0x3e2aaa49u), E4 = __uint_as_float(0x3d2aac79u);
+    const float E5 = __uint_as_float(0x3c091cf1u), E6 = __uint_as_float(0x3ab5121au);
+    const float t = __fmaf_rn(e, LOG2E, MAGIC);
+    const float nf = __fadd_rn(t, -MAGIC);
+    float r = __fmaf_rn(nf, NLN2_HI, e);
+    r = __fmaf_rn(nf, NLN2_LO, r);
+    float p = __fmaf_rn(E6, r, E5);
+    p = __fmaf_rn(p, r, E4);
+    p = __fmaf_rn(p, r, E3);
+    p = __fmaf_rn(p, r, E2);
+    p = __fmaf_rn(p, r, 1.0f);
+    p = __fmaf_rn(p, r, 1.0f);
+    const zi32 n = (zi32)(__float_as_uint(t) - 0x4b400000u);
+    const double dp = (double)p;
+    return __hiloint2double(__double2hiint(dp) + (n << 20), __double2loint(dp));
+}
+
+/* fast mode: the same split e*log2e = n + r, with 2^r from MUFU.EX2 */
+__device__ __forceinline__ double zmc_fexp_value(float e) {
+    if (!(fabsf(e) <= 708.0f)) {
+        if (e < 0.0f) return 0.0;
+        if (e > 0.0f) return __longlong_as_double(0x7FF0000000000000ll);
+        return __longlong_as_double(0x7FF8000000000000ll);
+    }
+    const float MAGIC = __uint_as_float(0x4b400000u);
+    const float y = __fmul_rn(e, __uint_as_float(0x3fb8aa3bu));
+    const float t = __fadd_rn(y, MAGIC);
+    const float nf = __fadd_rn(t, -MAGIC);
+    const float r = __fadd_rn(y, -nf);
+    float p;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(p) : "f"(r));
+    const zi32 n = (zi32)(__float_as_uint(t) - 0x4b400000u);
+    const double dp = (double)p;
+    return __hiloint2double(__double2hiint(dp) + (n << 20), __double2loint(dp));
+}
+
+/* ------------------------------------------------------------------ R2 + R4: cell geometry and the word -> point map */
+/* lo_d = lower_d + (double)I_d * width_d (multiply, then add).
+ * FP64: x = lo + ((double)w + 0.5) * (width * 2^-32).
+ * FP32: u' = bits(0x3F800000 | w>>9) in [1,2) ; x = fmaf(u', (float)width, base),
+ *       base = (float)(((lo - width) + width*2^-24) - centre), formed in FP64. */
+template <int D>
+struct ZmcMapF32 {
+    float wf[D], base[D];
+    __device__ __forceinline__ void init_dim(int d, double lower, double width, zu32 coord, double centre) {
+        const double lo = __dadd_rn(lower, __dmul_rn((double)coord, width));
+        double b = __dadd_rn(__dadd_rn(lo, -width), __dmul_rn(width, 5.9604644775390625e-08));
+        b = __dadd_rn(b, -centre);
+        base[d] = (float)b;
+        wf[d] = (float)width;
+    }
+    __device__ __forceinline__ float x(int d, zu32 w) const {
+        return __fmaf_rn(__uint_as_float(0x3F800000u | (w >> 9)), wf[d], base[d]);
+    }
+};
+
+template <int D>
+struct ZmcMapF64 {
+    double lo[D], step[D];
+    __device__ __forceinline__ void init_dim(int d, double lower, double width, zu32 coord) {
+        lo[d] = __dadd_rn(lower, __dmul_rn((double)coord, width));
+        step[d] = __dmul_rn(width, 2.3283064365386963e-10);
+    }
+    __device__ __forceinline__ double x(int d, zu32 w) const {
+        return __dadd_rn(lo[d], __dmul_rn(__dadd_rn(__uint2double_rn(w), 0.5), step[d]));
+    }
+};
+
+/* ------------------------------------------------------------------ integrands */
+/* Each integrand policy has
+ *   setup(args, instance, coords)  once per work item: geometry and this instance's parameters
+ *   eval(words, xout)              one sample from D consecutive words -> the FP64 value the unit sum adds
+ *                                  (xout != nullptr only in the debug kernel). */
+#ifdef ZMC_USER_FN
+__device__ float ZMC_USER_FN(const float* x, int dim, const float* p, int np);
+__device__ double ZMC_USER_FN(const double* x, int dim, const double* p, int np);
+#endif
+
+template <int ID, int D_, int PREC, int MODE>
+struct ZmcIntegrand;
+
+template <int ID, int D_, int MODE>
+struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
+    static constexpr int D = D_;
+    ZmcMapF32<D_> map;
+    float c0;           /* CONST/LINEAR: p[0] ; EXP_QUAD: -a */
+    float lin[ID == ZMC_ID_LINEAR ? D_ : 1];
+    const float* up;    /* user parameters */
+    zi32 unp;
+
+    __device__ __forceinline__ void setup(const ZmcSampleArgs& a, zu32 inst, const zu32* coords) {
+        const double* p = a.params + (zu64)inst * (zu64)a.ppi;
+#pragma unroll
+        for (int d = 0; d < D_; ++d) {
+            const double centre = (ID == ZMC_ID_EXP_QUAD) ? p[2 + d] : 0.0;
+            map.init_dim(d, a.lower[d], a.width[d], coords[d], centre);
+        }
+        c0 = 0.0f;
+        if (ID == ZMC_ID_CONST || ID == ZMC_ID_LINEAR) c0 = (float)p[0];
+        if (ID == ZMC_ID_EXP_QUAD) c0 = -(float)p[1];
+        if (ID == ZMC_ID_LINEAR) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) lin[d] = (float)p[1 + d];
+        }
+        up = a.params_f32 + (zu64)inst * (zu64)a.ppi;
+        unp = a.ppi;
+    }
+
+    __device__ __forceinline__ double eval(const zu32* w, double* xout) const {
+        float x[D_];
+#pragma unroll
+        for (int d = 0; d < D_; ++d) x[d] = map.x(d, w[d]);
+        if (xout) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) xout[d] = (double)x[d];
+        }
+        if (ID == ZMC_ID_CONST) return (double)c0;
+        if (ID == ZMC_ID_LINEAR) {
+            float f = c0;
+#pragma unroll
+            for (int d = 0; d < D_; ++d) f = __fmaf_rn(lin[d], x[d], f);
+            return (double)f;
+        }
+        if (ID == ZMC_ID_SIN_SUM) {          /* paper f1, Eq. (1) */
+            float s = x[0];
+#pragma unroll
+            for (int d = 1; d < D_; ++d) s = __fadd_rn(s, x[d]);
+            if (MODE == ZMC_MODE_FAST) return (double)__sinf(s);
+            return (double)zmc_zsin(s);
+        }
+        if (ID == ZMC_ID_EXP_QUAD) {         /* paper f2, Eq. (2); x holds x - c */
+            float q = __fmul_rn(x[0], x[0]);
+#pragma unroll
+            for (int d = 1; d < D_; ++d) q = __fmaf_rn(x[d], x[d], q);
+            const float e = __fmul_rn(c0, q);
+            if (MODE == ZMC_MODE_FAST) return zmc_fexp_value(e);
+            return zmc_zexp_value(e);
+        }
+#ifdef ZMC_USER_FN
+        if (ID == ZMC_ID_USER) return (double)ZMC_USER_FN((const float*)x, D_, up, unp);
+#endif
+        return 0.0;
+    }
+};
+
+template <int ID, int D_, int MODE>
+struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
+    static constexpr int D = D_;
+    ZmcMapF64<D_> map;
+    double c0;          /* CONST/LINEAR: p[0] ; EXP_QUAD: a */
+    double aux[(ID == ZMC_ID_LINEAR || ID == ZMC_ID_EXP_QUAD) ? D_ : 1];   /* LINEAR: coefficients ; EXP_QUAD: centre */
+    const double* up;
+    zi32 unp;
+
+    __device__ __forceinline__ void setup(const ZmcSampleArgs& a, zu32 inst, const zu32* coords) {
+        const double* p = a.params + (zu64)inst * (zu64)a.ppi;
+#pragma unroll
+        for (int d = 0; d < D_; ++d) map.init_dim(d, a.lower[d], a.width[d], coords[d]);
+        c0 = 0.0;
+        if (ID == ZMC_ID_CONST || ID == ZMC_ID_LINEAR) c0 = p[0];
+        if (ID == ZMC_ID_EXP_QUAD) c0 = p[1];
+        if (ID == ZMC_ID_LINEAR) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) aux[d] = p[1 + d];
+        }
+        if (ID == ZMC_ID_EXP_QUAD) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) aux[d] = p[2 + d];
+        }
+        up = p;
+        unp = a.ppi;
+    }
+
+    __device__ __forceinline__ double eval(const zu32* w, double* xout) const {
+        double x[D_];
+#pragma unroll
+        for (int d = 0; d < D_; ++d) x[d] = map.x(d, w[d]);
+        if (xout) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) xout[d] = x[d];
+        }
+        if (ID == ZMC_ID_CONST) return c0;
+        if (ID == ZMC_ID_LINEAR) {
+            double f = c0;
+#pragma unroll
+            for (int d = 0; d < D_; ++d) f = __dadd_rn(f, __dmul_rn(aux[d], x[d]));
+            return f;
+        }
+        if (ID == ZMC_ID_SIN_SUM) {
+            double s = x[0];
+#pragma unroll
+            for (int d = 1; d < D_; ++d) s = __dadd_rn(s, x[d]);
+            return sin(s);
+        }
+        if (ID == ZMC_ID_EXP_QUAD) {
+            double q = 0.0;
+#pragma unroll
+            for (int d = 0; d < D_; ++d) {
+                const double y = __dadd_rn(x[d], -aux[d]);
+                const double yy = __dmul_rn(y, y);
+                q = (d == 0) ? yy : __dadd_rn(q, yy);
+            }
+            return exp(-__dmul_rn(c0, q));
+        }
+#ifdef ZMC_USER_FN
+        if (ID == ZMC_ID_USER) return ZMC_USER_FN((const double*)x, D_, up, unp);
+#endif
+        return 0.0;
+    }
+};
+
+/* ------------------------------------------------------------------ work-item decoding (R2) */
+/* item -> (cell, trial, chunk); cell -> (parent G, child j); child j -> digits j_d (axis 0 least
+ * significant), I'_d = I_d*g + j_d ; path P' = P*k + j (80 bits). */
+template <int D>
+struct ZmcUnit {
+    zu32 inst, trial, chunk;
+    zu64 cell;
+    zu64 path_lo;
+    zu32 path_hi;
+    zu32 coords[D];
+    __device__ __forceinline__ void decode(const ZmcSampleArgs& a, zu64 item, zu32 n_chunks) {
+        const zu64 unit = item / n_chunks;
+        chunk = (zu32)(item - unit * n_chunks);
+        cell = unit / a.T;
+        trial = (zu32)(unit - cell * a.T);
+        const zu64 G = cell / a.k;
+        zu64 j = cell - G * a.k;
+        inst = a.par_inst[G];
+        const zu64 plo = a.par_plo[G];
+        const zu32 phi = a.par_phi[G];
+        path_lo = plo * a.k + j;
+        const zu64 carry = __umul64hi(plo, a.k) + ((path_lo < j) ? 1ull : 0ull);
+        path_hi = (zu32)((zu64)phi * a.k + carry);
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+            const zu64 jq = j / a.g;
+            const zu32 jd = (zu32)(j - jq * a.g);
+            j = jq;
+            coords[d] = a.par_coord[(zu64)d * a.par_stride + G] * a.g + jd;
+        }
+    }
+};
+
+/* ------------------------------------------------------------------ the fused sampling kernel */
+/* Flat word stream (R3): sample s, dimension d uses word s*D + d of the unit's stream; word i lives
+ * in Philox call i>>2, lane i&3. A "group" is the smallest run of samples that starts on a call
+ * boundary: SG = 4/gcd(D,4) samples = CG = D/gcd(D,4) calls. */
+template <int D> struct ZmcGroup {
+    static constexpr int G4 = (D % 4 == 0) ? 4 : ((D % 2 == 0) ? 2 : 1);
+    static constexpr int SG = 4 / G4;
+    static constexpr int CG = D / G4;
+};
+
+template <class F>
+__device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
+                                               double* acc) {
+    constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
+    zu32 w[4 * CG];
+    const zu32 q0 = gi * (zu32)CG;
+#pragma unroll
+    for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+#pragma unroll
+    for (int s = 0; s < SG; ++s) acc[s] = __dadd_rn(acc[s], f.eval(&w[s * D], nullptr));
+}
+
+template <class F>
+__global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZMC_MIN_BLOCKS) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
+    constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
+    const zu32 lane = threadIdx.x & 31u;
+    ZmcLevelInfo* const info = a.info;
+    const zu64 n_items = info->n_items;
+    const zu32 n_chunks = info->n_chunks;
+    const zu32 chunk_groups = info->chunk_groups;
+    const zu32 full_groups = (zu32)(a.N / (zu64)SG);       /* groups whose SG samples all exist */
+    const zu32 tail = (zu32)(a.N - (zu64)full_groups * SG); /* samples in the last, partial group */
+    const zu32 n_groups = full_groups + (tail ? 1u : 0u);
+
+    for (;;) {
+        zu64 item = 0;
+        if (lane == 0) item = atomicAdd(&info->work_ctr, 1ull);
+        item = __shfl_sync(0xFFFFFFFFu, item, 0);
+        if (item >= n_items) break;
+
+        ZmcUnit<D> u;
+        u.decode(a, item, n_chunks);
+        F f;
+        f.setup(a, u.inst, u.coords);
+        ZmcKeySchedule ks;
+        ks.init(a.keys[2 * u.inst], a.keys[2 * u.inst + 1]);
+        ZmcUnitCounter uc;
+        uc.init(u.path_lo, u.path_hi, a.level, u.trial);
+
+        const zu32 gb = u.chunk * chunk_groups;
+        const zu32 ge = (gb + chunk_groups < n_groups) ? gb + chunk_groups : n_groups;
+        const zu32 gfe = (ge < full_groups) ? ge : full_groups;
+
+        double acc[2 * SG];
+#pragma unroll
+        for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
+        zu32 gi = gb + lane;
+        for (; gi + 32u < gfe; gi += 64u) {
+            zmc_group_eval(f, ks, uc, gi, acc);
+            zmc_group_eval(f, ks, uc, gi + 32u, acc + SG);
+        }
+        if (gi < gfe) zmc_group_eval(f, ks, uc, gi, acc);
+        if (tail != 0u && ge > full_groups && lane == 0u) {   /* the partial group: only its first `tail` samples exist */
+            zu32 w[4 * CG];
+            const zu32 q0 = full_groups * (zu32)CG;
+#pragma unroll
+            for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+#pragma unroll
+            for (int s = 0; s < SG; ++s)
+                if ((zu32)s < tail) acc[s] = __dadd_rn(acc[s], f.eval(&w[s * D], nullptr));
+        }
+        double sum = acc[0];
+#pragma unroll
+        for (int s = 1; s < 2 * SG; ++s) sum = __dadd_rn(sum, acc[s]);
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
+        if (lane == 0u) a.partial[item] = sum;
+    }
+}
+
+/* Debug kernel (parity tests P1): the first n samples of one unit through the same device functions. */
+struct ZmcPointsArgs {
+    ZmcSampleArgs a;        /* geometry, keys, parameters; par_* and partial unused */
+    zu32 inst, trial;
+    zu64 path_lo;
+    zu32 path_hi;
+    zu32 coords[ZMC_DEV_MAX_DIM];
+    zu64 n;
+    double* x;              /* [n*D] */
+    double* f;              /* [n] */
+};
+
+template <class F>
+__global__ void zmc_points_kernel(const __grid_constant__ ZmcPointsArgs pa) {
+    constexpr int D = F::D;
+    F f;
+    zu32 coords[D];
+#pragma unroll
+    for (int d = 0; d < D; ++d) coords[d] = pa.coords[d];
+    f.setup(pa.a, pa.inst, coords);
+    ZmcKeySchedule ks;
+    ks.init(pa.a.keys[2 * pa.inst], pa.a.keys[2 * pa.inst + 1]);
+    ZmcUnitCounter uc;
+    uc.init(pa.path_lo, pa.path_hi, pa.a.level, pa.trial);
+    for (zu64 s = (zu64)blockIdx.x * blockDim.x + threadIdx.x; s < pa.n; s += (zu64)gridDim.x * blockDim.x) {
+        zu32 w[D];
+        zu32 cur[4];
+        zu64 have = ~0ull;
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+            const zu64 idx = s * (zu64)D + (zu64)d;
+            if ((idx >> 2) != have) { have = idx >> 2; zmc_philox((zu32)have, uc.c1, uc.c2, uc.c3, ks, cur); }
+            w[d] = cur[idx & 3ull];
+        }
+        double xo[D];
+        const double v = f.eval(w, xo);
+        if (pa.f) pa.f[s] = v;
+        if (pa.x) {
+#pragma unroll
+            for (int d = 0; d < D; ++d) pa.x[s * D + d] = xo[d];
+        }
+    }
+}
+
+#endif /* ZMC_DEVICE_CUH */

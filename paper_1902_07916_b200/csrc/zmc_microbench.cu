@@ -1,0 +1,161 @@
+/*
+ * zmc_microbench.cu -- issue-rate microbenchmarks of the pipes the sampling kernel uses.
+ * They give the denominator of the ALU roofline: the path is bound by the
+ * warp schedulers' issue slots and the integer pipes (Philox is 20 IMAD.WIDE.U32 + 20 LOP3 per
+ * call), not by HBM, the tensor cores or the SFU, so the peak has to come from measured
+ * instruction throughput, not from a data sheet.
+ *
+ * Each kernel runs a long unrolled loop of the instruction under test on ILP independent chains
+ * per thread, 4 CTAs of 256 threads per SM (8 warps per scheduler, one wave), and reports
+ * warp-instructions / SM / clock with the clock taken from clock64() on every SM.
+ */
+#include <cuda_runtime.h>
+
+#include "../../include/zmc.h"
+#include "zmc_device.cuh"
+
+namespace {
+
+constexpr int kIters = 4096;
+constexpr int kIlp = 8;
+
+template <int WHICH>
+__global__ void __launch_bounds__(256, 4) mb_kernel(zu32* sink, unsigned long long* cycles, zu32 seed) {
+    const long long t0 = clock64();
+    zu32 r[kIlp];
+    float f[kIlp];
+    double d[kIlp];
+#pragma unroll
+    for (int i = 0; i < kIlp; ++i) {
+        r[i] = seed + threadIdx.x * 977u + i * 131u;
+        f[i] = __uint_as_float(0x3f800000u | (r[i] & 0xFFFFu));
+        d[i] = (double)f[i];
+    }
+    zu32 acc = 0;
+    const zu32 k0 = seed * 3u + 1u, k1 = seed * 5u + 7u;
+    const float fc = __uint_as_float(0x3f7ff000u | (seed & 0xFFu));
+    const double dc = (double)fc;
+#pragma unroll 1
+    for (int it = 0; it < kIters; ++it) {
+#pragma unroll
+        for (int i = 0; i < kIlp; ++i) {
+            if (WHICH == 0) {            /* IMAD.WIDE.U32: 32x32 -> 64, both halves consumed by the next one */
+                const zu64 p = (zu64)r[i] * (zu64)ZMC_PHILOX_M0;
+                zu32 lo, hi;
+                asm volatile("mov.b64 {%0,%1}, %2;" : "=r"(lo), "=r"(hi) : "l"(p));
+                asm volatile("" : "+r"(lo), "+r"(hi));
+                r[i] = hi;
+                acc += 0;   /* lo is dead on purpose: one instruction per step */
+                (void)lo;
+            } else if (WHICH == 1) {     /* LOP3 (3-input xor) */
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[i]) : "r"(k0), "r"(k1));
+            } else if (WHICH == 2) {     /* Philox round mix: IMAD.WIDE.U32 + LOP3 */
+                const zu64 p = (zu64)r[i] * (zu64)ZMC_PHILOX_M0;
+                const zu32 lo = (zu32)p, hi = (zu32)(p >> 32);
+                asm volatile("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r[i]) : "r"(hi), "r"(lo), "r"(k0));
+            } else if (WHICH == 3) {     /* FFMA */
+                asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[i]) : "f"(fc), "f"(f[(i + 1) % kIlp]));
+            } else if (WHICH == 4) {     /* FADD */
+                asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(fc));
+            } else if (WHICH == 5) {     /* DADD */
+                asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(d[i]) : "d"(dc));
+            } else if (WHICH == 6) {     /* F2F.F64.F32 (+ F2F.F32.F64 back would double count: use a float source chain) */
+                double t;
+                asm volatile("cvt.f64.f32 %0, %1;" : "=d"(t) : "f"(f[i]));
+                d[i] = t;
+                asm volatile("" : "+f"(f[i]));
+            } else if (WHICH == 7) {     /* MUFU.SIN */
+                asm volatile("sin.approx.ftz.f32 %0, %0;" : "+f"(f[i]));
+            } else if (WHICH == 8) {     /* MUFU.EX2 */
+                asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(f[i]));
+            } else if (WHICH == 9) {     /* DFMA */
+                asm volatile("fma.rn.f64 %0, %0, %1, %1;" : "+d"(d[i]) : "d"(dc));
+            } else if (WHICH == 11) {    /* I2F.F64.U32 */
+                double t;
+                asm volatile("cvt.rn.f64.u32 %0, %1;" : "=d"(t) : "r"(r[i]));
+                d[i] = t;
+                asm volatile("" : "+r"(r[i]));
+            } else if (WHICH == 12) {    /* LEA.HI-like: (w >> 9) | 0x3F800000 */
+                asm volatile("{ .reg .b32 t; shr.u32 t, %0, 9; or.b32 %0, t, 0x3F800000; }" : "+r"(r[i]));
+            }
+        }
+        if (WHICH == 10) {               /* whole Philox4x32-10 calls, kIlp/2 independent calls per step */
+            ZmcKeySchedule ks;
+            ks.init(k0, k1);
+#pragma unroll
+            for (int i = 0; i < kIlp / 2; ++i) {
+                zu32 w[4];
+                zmc_philox(r[i] + (zu32)it, r[i + 1], k0, k1, ks, w);
+                r[i] ^= w[0] ^ w[1] ^ w[2] ^ w[3];
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < kIlp; ++i) acc ^= r[i] ^ __float_as_uint(f[i]) ^ (zu32)__double2loint(d[i]) ^ (zu32)__double2hiint(d[i]);
+    const long long t1 = clock64();
+    if (acc == 0x12345678u) sink[0] = acc;
+    if (threadIdx.x == 0) atomicMax(cycles, (unsigned long long)(t1 - t0));
+}
+
+template <int W>
+cudaError_t launch(int grid, zu32* sink, unsigned long long* cyc, cudaStream_t st) {
+    mb_kernel<W><<<grid, 256, 0, st>>>(sink, cyc, 12345u);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, double* sm_mhz) {
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return ZMC_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return ZMC_ERR_CUDA;
+    const int grid = sms * 4;
+    zu32* sink = nullptr;
+    unsigned long long* cyc = nullptr;
+    if (cudaMalloc(&sink, 256) != cudaSuccess || cudaMalloc(&cyc, 8) != cudaSuccess) return ZMC_ERR_CUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaError_t e = cudaSuccess;
+    float ms = 0.f;
+    unsigned long long hc = 0;
+    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   /* the last repetition is the measurement */
+        cudaMemsetAsync(cyc, 0, 8, st);
+        cudaEventRecord(e0, st);
+        switch (which) {
+            case 0: e = launch<0>(grid, sink, cyc, st); break;
+            case 1: e = launch<1>(grid, sink, cyc, st); break;
+            case 2: e = launch<2>(grid, sink, cyc, st); break;
+            case 3: e = launch<3>(grid, sink, cyc, st); break;
+            case 4: e = launch<4>(grid, sink, cyc, st); break;
+            case 5: e = launch<5>(grid, sink, cyc, st); break;
+            case 6: e = launch<6>(grid, sink, cyc, st); break;
+            case 7: e = launch<7>(grid, sink, cyc, st); break;
+            case 8: e = launch<8>(grid, sink, cyc, st); break;
+            case 9: e = launch<9>(grid, sink, cyc, st); break;
+            case 10: e = launch<10>(grid, sink, cyc, st); break;
+            case 11: e = launch<11>(grid, sink, cyc, st); break;
+            case 12: e = launch<12>(grid, sink, cyc, st); break;
+            default: e = cudaErrorInvalidValue;
+        }
+        cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess) e = cudaMemcpy(&hc, cyc, 8, cudaMemcpyDeviceToHost);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    cudaFree(cyc);
+    if (e != cudaSuccess) return which < 0 || which > 12 ? ZMC_ERR_ARG : ZMC_ERR_CUDA;
+    /* per thread: kIters * kIlp instructions (which 2: 2 each ; which 10: kIlp/2 Philox calls per step) */
+    double per_thread = (double)kIters * kIlp;
+    if (which == 2) per_thread *= 2.0;
+    if (which == 10) per_thread = (double)kIters * (kIlp / 2);
+    const double warps_per_sm = 4.0 * 256.0 / 32.0;
+    /* all CTAs of an SM are resident at once (4 x 256 threads), so the SM's elapsed clocks ~ the longest CTA */
+    if (per_sm_clk) *per_sm_clk = per_thread * warps_per_sm / (double)hc;
+    if (sm_mhz) *sm_mhz = (double)hc / (ms * 1e3);
+    return ZMC_OK;
+}
