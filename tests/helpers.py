@@ -65,3 +65,69 @@ def var_sin_sum_box(lower, upper) -> float:
 
 def ulp32(x) -> float:
     return float(np.spacing(np.float32(abs(x))))
+
+
+# ---------------------------------------------------------------- GPU-vs-oracle comparison (parity rules P2-P4)
+def compare_tree(it, ores, w: W.Workload, *, tol_sum=1e-12, tol_stat=1e-11, exact_sets=True):
+    """Compare every level of a finished CUDA run `it` (binding.Integrator, keep_level_stats on) with
+    the oracle result `ores` (oracle.run(..., keep_cells=True)) cell by cell.
+
+    P2  per-(cell,trial) sums: |S_gpu - S_orc| <= tol_sum * N (|f| <= 1 for the bounded built-ins;
+        callers with unbounded f pass a scaled tol_sum) -- only the FP64 summation order differs.
+    P3  refined sets identical (exact mode).
+    P4  value/std: relative 1e-6 is BASELINE.json's bar; tol_stat is what exact mode achieves.
+    Returns the number of cells compared."""
+    st = it.stats()
+    n_cmp = 0
+    assert st.overflow == 0
+    for lev, ol in enumerate(ores.levels, start=1):
+        gl = it.level_cells(lev)
+        assert len(gl.mu) == ol.n_cells, (lev, len(gl.mu), ol.n_cells)
+        assert st.level[lev - 1].n_cells == ol.n_cells
+        assert st.level[lev - 1].n_refined == ol.n_refined
+        np.testing.assert_array_equal(gl.instance, ol.instance)
+        assert gl.path == ol.path
+        scale = float(w.n_samples)
+        dS = np.abs(gl.S - ol.S)
+        assert dS.max() <= tol_sum * scale, (lev, dS.max())
+        sc = max(np.abs(ol.mu).max(), ol.s.max(), 1e-300)
+        assert np.abs(gl.mu - ol.mu).max() <= tol_stat * sc
+        assert np.abs(gl.s - ol.s).max() <= 100 * tol_stat * sc
+        assert np.abs(gl.tau - ol.tau).max() <= 100 * tol_stat * max(ol.tau.max(), 1e-300)
+        if exact_sets:
+            np.testing.assert_array_equal(gl.refined, ol.refined)
+        n_cmp += ol.n_cells
+    for lev in range(len(ores.levels) + 1, w.depth + 1):   # levels the tree never reached
+        assert st.level[lev - 1].n_cells == 0
+    v, s = it.result()
+    assert np.all(np.abs(v - ores.value) <= 1e-6 * np.maximum(np.abs(ores.value), 1e-300))
+    assert np.all(np.abs(v - ores.value) <= tol_stat * np.maximum(np.abs(ores.value), ores.std))
+    assert np.all(np.abs(s - ores.std) <= 1e-9 * np.maximum(ores.std, 1e-300))
+    return n_cmp
+
+
+def host_control(mu, s, k, level, depth, m, instance, budget=0):
+    """Re-derive the control path (H7-H10) of one level in numpy from dumped per-cell (mu, s):
+    per-group tau = mean + m*pstd (R6), flags s > tau for level < depth (R7), first-B budget per
+    instance in path order (R12), accepted sums. Test-side restatement; shares nothing with either
+    implementation. Returns (tau_per_cell, refined, acc_value[instance], acc_var[instance])."""
+    n = len(mu)
+    G = n // k
+    sg = s.reshape(G, k)
+    mean = sg.mean(axis=1)
+    pstd = np.sqrt(((sg - mean[:, None]) ** 2).mean(axis=1))
+    tau = mean + m * pstd
+    tau_c = np.repeat(tau, k)
+    flag = (s > tau_c) & (level < depth)
+    refined = flag.copy()
+    if budget > 0:
+        for b in np.unique(instance):
+            idx = np.nonzero(flag & (instance == b))[0]
+            refined[idx[budget:]] = False
+    ninst = int(instance.max()) + 1
+    val = np.zeros(ninst)
+    var = np.zeros(ninst)
+    acc = ~refined
+    np.add.at(val, instance[acc], mu[acc])
+    np.add.at(var, instance[acc], s[acc] ** 2)
+    return tau_c, refined, val, var

@@ -1,0 +1,87 @@
+"""CPU-side checks of the boundary (no compute calls): libzmc.so builds for sm_100a, loads, exports every
+symbol include/zmc.h declares, validates arguments, and refuses to work without a CUDA device
+(there is no CPU fallback; the oracle is never reachable from the product)."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1902_07916_b200 import binding as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "zmc.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(zmc_[a-z_]+)\s*\(", text)))
+
+
+def test_header_symbols_all_exported():
+    L = B.lib()
+    names = _declared()
+    assert set(names) == set(B.EXPORTS), (names, B.EXPORTS)
+    for n in names:
+        assert getattr(L, n) is not None
+
+
+def test_library_is_sm100a_only_and_has_no_oracle_symbols():
+    out = subprocess.run(["cuobjdump", "-lelf", B.LIB_PATH], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, archs
+    syms = subprocess.run(["nm", "-D", "--defined-only", B.LIB_PATH], capture_output=True, text=True).stdout
+    assert "orc_" not in syms
+    # the product never imports the oracle
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_1902_07916_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "zmc_oracle" not in src, f
+
+
+def test_create_validates_arguments():
+    L = B.lib()
+    lo = np.zeros(3)
+    up = np.ones(3)
+    dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+
+    def create(dim=3, lower=lo, upper=up, g=4, N=100, T=5, depth=2, m=1.5, seed=1):
+        h = C.c_void_p()
+        rc = L.zmc_create(C.byref(h), dim, dp(lower) if lower is not None else None, dp(upper) if upper is not None else None,
+                          g, N, T, depth, m, seed)
+        msg = L.zmc_last_error(h).decode() if h else ""
+        if h:
+            L.zmc_destroy(h)
+        return rc, msg
+
+    assert create(dim=0)[0] == B.ERR_ARG
+    assert create(lower=None)[0] == B.ERR_ARG
+    assert create(g=0)[0] == B.ERR_ARG
+    assert create(N=0)[0] == B.ERR_ARG
+    assert create(T=0)[0] == B.ERR_ARG
+    assert create(depth=0)[0] == B.ERR_ARG
+    assert create(m=float("nan"))[0] == B.ERR_ARG
+    assert create(upper=np.array([1.0, 0.0, 1.0]))[0] == B.ERR_ARG
+    assert create(upper=np.array([1.0, np.inf, 1.0]))[0] == B.ERR_ARG
+    rc, msg = create(T=256)
+    assert rc == B.ERR_RANGE and "255" in msg
+    assert create(depth=16)[0] == B.ERR_RANGE
+    assert create(dim=17, lower=np.zeros(17), upper=np.ones(17))[0] == B.ERR_RANGE
+    assert create(N=2 ** 33)[0] == B.ERR_RANGE                          # N*D/4 >= 2^32
+    assert create(dim=12, lower=np.zeros(12), upper=np.ones(12), g=4, depth=4)[0] == B.ERR_RANGE   # 96-bit path
+    assert create(g=70000, depth=2)[0] == B.ERR_RANGE                   # g^depth > 2^32
+    assert L.zmc_create(None, 3, dp(lo), dp(up), 4, 100, 5, 2, 1.5, 1) == B.ERR_ARG
+    assert L.zmc_status_string(B.ERR_CAPACITY).decode() == "level capacity exceeded"
+
+
+def test_no_device_means_error_not_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(B.ZmcError) as e:
+        B.Integrator(3, [0.0] * 3, [1.0] * 3, 4, 100, 5, 2, 1.5, 1)
+    assert e.value.status == B.ERR_CUDA
+    assert B.lib().zmc_microbench(0, None, None, None) == B.ERR_CUDA

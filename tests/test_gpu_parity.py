@@ -1,0 +1,290 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI of include/zmc.h, via the ctypes binding)
+against the oracle, element by element on the same seeded inputs (parity rules P1-P4, DESIGN.md
+section 5). Every test here needs a B200 and is marked gpu.
+
+Tolerances (derived from the arithmetic):
+  * Philox words, FP32 points and FP32 integrand values: bit-exact (integer work / the same IEEE
+    operation sequence on both sides, R8).
+  * FP64 points: bit-exact (same +,* sequence); FP64 sin/exp values: <= 4 ulp (libm vs CUDA libdevice).
+  * per-(cell,trial) sums: BASELINE.json asks 1e-6 relative; only the FP64 summation order differs,
+    so exact mode is held to 1e-12 * N (N terms each <= 1 in magnitude, error <= N * 2^-53 * log-ish).
+  * refined-cell sets: identical. Final integral: 1e-6 relative (BASELINE.json), in fact ~1e-13.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1902_07916_b200 import binding as B
+from paper_1902_07916_b200 import workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+def _run_both(w, math=B.MATH_EXACT, max_cells=1 << 18):
+    it = B.from_workload(w, math=math, keep_level_stats=True, max_cells_per_level=max_cells)
+    it.run()
+    ores = O.run(H.oracle_config(w), keep_cells=True)
+    return it, ores
+
+
+# ------------------------------------------------------------------ P1: generator, map, integrand
+def test_philox_words_bit_exact():
+    w = W.config4(n_instances=5)
+    with B.from_workload(w) as it:
+        cases = [(0, 0, 1, 0, 0, 4096), (3, 12345, 2, 4, 17, 1001), (4, (1 << 79) + (1 << 64) + 99, 15, 254, 3, 515),
+                 (1, (1 << 64) - 1, 7, 1, (1 << 33) + 2, 64), (2, 0x0123456789ABCDEF, 3, 2, 4 * ((1 << 32) - 8), 32)]
+        for inst, path, level, trial, first, n in cases:
+            g = it.debug_words(inst, path, level, trial, first, n)
+            o = O.unit_words(w.seed, inst, path, level, trial, first, n)
+            np.testing.assert_array_equal(g, o)
+
+
+@pytest.mark.parametrize("name", ["sin6_f32", "gauss9_f32", "gauss4_f32_batched", "linear5_f32", "const2_f32",
+                                  "sin3_f64", "gauss9_f64", "linear7_f64"])
+def test_points_and_values(name):
+    rng = np.random.default_rng(11)
+    if name == "sin6_f32":
+        w = W.config2()
+    elif name == "gauss9_f32":
+        w = W.config3()
+    elif name == "gauss4_f32_batched":
+        w = W.config4(n_instances=3)
+    elif name == "linear5_f32":
+        w = W.Workload("lin5", 5, (-1.0, 0.0, 2.0, -3.0, 0.5), (1.0, 0.25, 7.0, -1.0, 0.75), 3, 100, 3, 3, 1.5, 9,
+                       W.LINEAR, W.F32, params=rng.normal(size=(1, 6)))
+    elif name == "const2_f32":
+        w = W.Workload("c2", 2, (0.0, 0.0), (1.0, 2.0), 2, 10, 2, 1, 1.5, 9, W.CONST, W.F32, params=np.array([[0.3]]))
+    elif name == "sin3_f64":
+        w = W.config1()
+    elif name == "gauss9_f64":
+        w = W.config3().with_(precision=W.F64)
+    else:
+        w = W.Workload("lin7", 7, (0.0,) * 7, (1.0, 2.0, 3.0, 4.0, 5.0, 6.0, 7.0), 2, 100, 3, 3, 1.5, 9,
+                       W.LINEAR, W.F64, params=rng.normal(size=(1, 8)))
+    cfg = H.oracle_config(w)
+    n = 999
+    with B.from_workload(w) as it:
+        for level in (1, w.depth):
+            digits = [int(rng.integers(0, w.k)) for _ in range(level)]
+            if name.startswith("gauss9"):
+                digits = [(w.k - 1) // 2] * level      # the centre cell, where the values are not all zero
+            path, coords = O.path_coords(w.dim, w.g, digits)
+            inst = w.n_instances - 1
+            trial = w.trials - 1
+            xg, fg = it.debug_points(inst, path, level, coords, trial, n)
+            xo, fo = O.unit_points(cfg, inst, path, level, coords, trial, n)
+            np.testing.assert_array_equal(xg, xo)
+            if w.precision == W.F32 or w.integrand in (W.CONST, W.LINEAR):
+                np.testing.assert_array_equal(fg, fo)
+            else:
+                assert np.all(np.abs(fg - fo) <= 4 * np.spacing(np.abs(fo)))
+            if name.startswith("gauss9") and level > 1:
+                assert np.count_nonzero(fo) > n // 2
+
+
+def test_fast_mode_values_close():
+    """MUFU mode (R8): not bit-comparable; |sin| error <= 2^-21.4 on [-pi,pi] scaled by the range
+    reduction inside __sinf (abs error <= 4e-6 measured for |a| <= 60, bound 1e-5); exp relative error <= 1e-6."""
+    for w, tol in ((W.config2(), 1e-5), (W.config4(n_instances=2), 2e-6)):
+        cfg = H.oracle_config(w)
+        path, coords = O.path_coords(w.dim, w.g, [w.k // 3])
+        with B.from_workload(w, math=B.MATH_FAST) as it:
+            xg, fg = it.debug_points(0, path, 1, coords, 0, 2000)
+        xo, fo = O.unit_points(cfg, 0, path, 1, coords, 0, 2000)
+        np.testing.assert_array_equal(xg, xo)
+        if w.integrand == W.SIN_SUM:
+            assert np.abs(fg - fo).max() <= tol
+        else:
+            # e*log2(e) is rounded once in FP32 before MUFU.EX2: relative error ~ |e| * 2^-24 on top of EX2's 2^-22
+            assert np.all(np.abs(fg - fo) <= (tol + 1.5e-7 * np.abs(np.log(fo))) * np.abs(fo))
+
+
+# ------------------------------------------------------------------ P2-P4: whole trees, small enough for the oracle
+def test_config1_whole_tree():
+    """BASELINE.json configs[0] end to end, all 64 + 5*64 cells, 1920 (cell,trial) sums."""
+    w = W.config1()
+    it, ores = _run_both(w)
+    n = H.compare_tree(it, ores, w)
+    assert n == 64 + 5 * 64
+    assert sorted(np.nonzero(it.level_cells(1).refined)[0].tolist()) == [1, 24, 26, 34, 41]   # golden/config1_worked.txt
+    v, s = it.result()
+    closed = H.closed_sin_sum(w.lower, w.upper)
+    assert abs(v[0] - closed) <= 4 * s[0]
+    it.close()
+
+
+SMALL = {
+    # 6-D sin, FP32 exact: several tiles of cells, ragged sample count (N odd: last group half full), budget
+    "sin6_f32_ragged": W.config2().with_(n_samples=501, depth=2, max_groups_per_level=3),
+    # 9-D Gaussian, FP32 extended range: one refined cell per level, depth 3
+    "gauss9_f32": W.config3().with_(n_samples=203, depth=3),
+    # batched 4-D Gaussians: 6 instances, own keys / thresholds / budgets
+    "gauss4_batched": W.config4(n_instances=6).with_(n_samples=130, max_groups_per_level=2),
+    # FP64 Gaussian, D=2, deep tree without budget
+    "gauss2_f64_deep": W.Workload("g2", 2, (-1.0, -2.0), (1.5, 1.0), 3, 97, 4, 5, 0.5, 21, W.EXP_QUAD, W.F64,
+                                  params=np.array([[2.0, 40.0, 0.1, -0.3]])),
+    # D=1 and D=4 (a whole Philox call per sample), D=5 (4 samples per 5 calls), D=7, D=12
+    "sin1_f32": W.Workload("s1", 1, (0.0,), (3.0,), 7, 1001, 6, 3, 1.0, 5, W.SIN_SUM, W.F32),
+    "sin4_f64": W.Workload("s4", 4, (0.0,) * 4, (2.0,) * 4, 3, 63, 3, 2, 1.0, 6, W.SIN_SUM, W.F64),
+    "sin5_f32": W.Workload("s5", 5, (0.0,) * 5, (4.0,) * 5, 3, 1022, 5, 2, 1.5, 7, W.SIN_SUM, W.F32, max_groups_per_level=2),
+    "sin7_f32": W.Workload("s7", 7, (0.0,) * 7, (4.0,) * 7, 2, 333, 5, 3, 1.0, 8, W.SIN_SUM, W.F32, max_groups_per_level=5),
+    "lin12_f32": W.Workload("l12", 12, (0.0,) * 12, (1.0,) * 12, 2, 17, 3, 2, 1.0, 9, W.LINEAR, W.F32,
+                            params=np.linspace(-1, 1, 13)[None, :], max_groups_per_level=1),
+    # long units: N large enough that a unit is split into sample chunks (few cells, many samples)
+    "sin3_f64_chunks": W.Workload("s3c", 3, (0.0,) * 3, (10.0,) * 3, 2, 200003, 4, 2, 0.0, 10, W.SIN_SUM, W.F64),
+    "sin6_f32_chunks": W.Workload("s6c", 6, (0.0,) * 6, (10.0,) * 6, 1, 1000001, 3, 1, 1.5, 12, W.SIN_SUM, W.F32),
+}
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_small_whole_trees(name):
+    w = SMALL[name]
+    it, ores = _run_both(w)
+    H.compare_tree(it, ores, w)
+    if w.integrand == W.EXP_QUAD:   # sums span hundreds of decades: also compare each sum relative to itself (f >= 0)
+        for lev, ol in enumerate(ores.levels, start=1):
+            gl = it.level_cells(lev)
+            assert np.all(np.abs(gl.S - ol.S) <= 1e-12 * np.abs(ol.S))
+    it.close()
+
+
+def test_path_beyond_64_bits():
+    """D=11, g=2, depth 7: paths reach 77 bits (R2: 80-bit path in the Philox counter)."""
+    w = W.Workload("deep11", 11, (0.0,) * 11, (1.0,) * 11, 2, 8, 3, 7, 0.0, 13, W.LINEAR, W.F32,
+                   params=np.linspace(0.5, 2, 12)[None, :], max_groups_per_level=1)
+    it, ores = _run_both(w)
+    H.compare_tree(it, ores, w)
+    assert len(ores.levels) == 7 and max(ores.levels[6].path) >= 1 << 64
+    it.close()
+
+
+def test_fast_mode_whole_tree_within_bj_tolerance():
+    """P2 in fast mode: sums within 1e-6 relative to sum|f| <= N; P3/P4 as far as fast mode allows:
+    a refined-set difference is tolerated only for cells within the propagated deviation of tau."""
+    w = W.config2().with_(n_samples=2000, depth=2, max_groups_per_level=2)
+    it = B.from_workload(w, math=B.MATH_FAST, keep_level_stats=True, max_cells_per_level=1 << 16)
+    it.run()
+    ores = O.run(H.oracle_config(w), keep_cells=True)
+    g1, o1 = it.level_cells(1), ores.levels[0]
+    assert np.abs(g1.S - o1.S).max() <= 1e-6 * w.n_samples
+    diff = np.nonzero(g1.refined != o1.refined)[0]
+    V = (10.0 / 4) ** 6
+    delta = np.abs(g1.S - o1.S).max(axis=1) * V / w.n_samples + np.abs(g1.tau - o1.tau)
+    for c in diff:
+        assert abs(o1.s[c] - o1.tau[c]) <= 4 * delta[c] + 1e-6 * o1.tau[c]
+    if len(diff) == 0:
+        # every unit sum is within 1e-6 * sum|f| <= 1e-6 * N, so the integral is within 1e-6 * Vol * max|f|
+        # (the signed value suffers cancellation: -122 on a domain of volume 1e6); observed ~1e-9 * Vol
+        v, s = it.result()
+        assert abs(v[0] - ores.value[0]) <= 1e-6 * 10.0 ** 6
+        assert abs(v[0] - ores.value[0]) <= 1e-4 * ores.std[0]
+    it.close()
+
+
+# ------------------------------------------------------------------ degenerate cases (R7)
+def test_degenerate_cases():
+    # CONST: every s is 0 -> tau = 0 -> nothing flagged (0 > 0 is false); value = c * Vol; std = 0
+    w = W.Workload("c3", 3, (0.0, 1.0, -1.0), (2.0, 3.0, 1.0), 3, 50, 4, 3, 1.5, 1, W.CONST, W.F64, params=np.array([[0.75]]))
+    it, ores = _run_both(w)
+    H.compare_tree(it, ores, w)
+    v, s = it.result()
+    assert abs(v[0] - 0.75 * 8.0) < 1e-12 and s[0] == 0.0
+    assert it.stats().level[1].n_cells == 0
+    it.close()
+    # g = 1 (k = 1): one cell per group, s = tau, never flagged; T = 1: every s = 0; N = 1; depth 1
+    for kw in (dict(g=1, depth=3), dict(trials=1, depth=3), dict(n_samples=1, depth=2), dict(depth=1),
+               dict(n_samples=3, depth=2)):
+        w = W.config1().with_(**kw)
+        it, ores = _run_both(w)
+        H.compare_tree(it, ores, w)
+        it.close()
+
+
+def test_nan_is_accepted_and_counted():
+    """R7: NaN s compares false -> accepted; result NaN; counted in zmc_stats.nonfinite."""
+    w = W.Workload("nan", 2, (0.0, 0.0), (1.0, 1.0), 2, 16, 3, 2, 1.0, 1, W.CONST, W.F64, params=np.array([[np.nan]]))
+    with B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 12) as it:
+        it.run()
+        v, s = it.result()
+        assert np.isnan(v[0])
+        st = it.stats()
+        assert st.nonfinite == 4 and st.level[0].n_refined == 0
+
+
+def test_capacity_overflow_is_reported():
+    w = W.config1().with_(sigma_multiplier=-10.0, depth=3)     # tau below every s: all 64 cells flagged
+    with B.from_workload(w, max_cells_per_level=64 * 8) as it:  # room for 8 parents only
+        it.run()
+        with pytest.raises(B.ZmcError) as e:
+            it.result()
+        assert e.value.status == B.ERR_CAPACITY
+        assert it.stats().overflow == 1
+
+
+def test_rerun_is_bit_identical_and_workspace_from_torch():
+    import torch
+    w = W.config1()
+    with B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 12) as it:
+        it.use_torch_workspace()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            it.run()
+            a = it.result()
+            c1 = it.level_cells(2)
+            it.run()
+            b = it.result()
+            c2 = it.level_cells(2)
+        assert a[0][0] == b[0][0] and a[1][0] == b[1][0]
+        np.testing.assert_array_equal(c1.S, c2.S)
+        np.testing.assert_array_equal(c1.mu, c2.mu)
+
+
+# ------------------------------------------------------------------ user integrand (NVRTC, sm_100a)
+USER_SRC = r"""
+__device__ double my_f(const double* x, int dim, const double* p, int np) {
+    double a = 0.0;
+    for (int d = 0; d < dim; ++d) a += x[d];
+    return p[0] * sin(a);
+}
+__device__ float my_f(const float* x, int dim, const float* p, int np) {
+    float a = 0.0f;
+    for (int d = 0; d < dim; ++d) a += x[d];
+    return p[0] * sinf(a);
+}
+"""
+
+
+def test_user_integrand_jit():
+    w = W.config1()
+    closed = 2.0 * H.closed_sin_sum(w.lower, w.upper)
+    for prec in (B.F64, B.F32):
+        it = B.Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
+        it.set_option(B.OPT_PRECISION, prec)
+        it.set_integrand_source(USER_SRC, "my_f", np.array([[2.0]]), 1)
+        it.set_option(B.OPT_KEEP_LEVEL_STATS, 1)
+        it.set_option(B.OPT_MAX_CELLS_PER_LEVEL, 1 << 12)
+        it.run()
+        v, s = it.result()
+        assert abs(v[0] - closed) <= 4 * s[0]
+        if prec == B.F64:   # same points, same sums as the built-in up to the factor 2 and sin's last ulp
+            ores = O.run(H.oracle_config(w), keep_cells=True)
+            g1 = it.level_cells(1)
+            assert np.abs(g1.S - 2.0 * ores.levels[0].S).max() <= 1e-10 * w.n_samples
+            np.testing.assert_array_equal(g1.refined, ores.levels[0].refined)
+        it.close()
+    it = B.Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
+    with pytest.raises(B.ZmcError) as e:
+        it.set_integrand_source("__device__ double broken(const double* x, int d, const double* p, int n) { return y; }",
+                                "broken", None, 1)
+    assert e.value.status == B.ERR_COMPILE and "error" in str(e.value)
+    it.close()
+
+
+def test_dimension_above_aot_range_is_jitted():
+    """13 <= D <= 16 has no pre-compiled kernel: the built-in is JIT-compiled from the same device source."""
+    w = W.Workload("l13", 13, (0.0,) * 13, (1.0,) * 13, 1, 64, 3, 1, 1.0, 3, W.LINEAR, W.F32,
+                   params=np.linspace(-1, 1, 14)[None, :])
+    it, ores = _run_both(w)
+    H.compare_tree(it, ores, w)
+    it.close()
