@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- integrand evaluations per second of the whole hot path on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--math exact|fast] [--impl reference]
+
+A "step" is one complete tree search (zmc_run: every level's sampling + control kernels) of the
+workload; inputs (bounds, parameters, derived keys) are resident on the device for `value`, and pass
+through the C ABI from host arrays, with the result read back, for `e2e`. One JSON line on stdout.
+DESIGN.md section 7 states the workloads, the ALU roofline and what each key means.
+
+N > 1 (torchrun, one rank per GPU): BASELINE.json rules multi-GPU out of scope ("one GPU only"), so
+the ranks are independent replicas of the same problem with seeds seed+rank -- no data-path
+collective; torch.distributed only supplies the barrier, the max over ranks of the device time and
+the sum of evaluations ("scaling": "weak").
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "integrand_evals_per_s"
+UNIT = "evals/s"
+PHILOX_IMAD_WIDE_PER_CALL = 20      # 2 IMAD.WIDE.U32 per round, 10 rounds
+IMAD_WIDE_CLK_PER_WARP_INST_PER_SM = 1.0   # measured on B200 (zmc_microbench which=0/10), DESIGN.md section 6
+
+
+def workloads():
+    from paper_1902_07916_b200 import workloads as W
+    return {
+        # BASELINE.json configs[1] with the refinement budget of DESIGN.md R12 (paper semantics need 2.2e14 evals)
+        "cfg2_sin6d_depth3_B16": W.config2(depth=3, budget=16),
+        # BASELINE.json configs[1], levels 1-2 with the budget off (paper semantics; 6.4e11 evals, ~3 s per step)
+        "cfg2_sin6d_depth2": W.config2(depth=2, budget=0),
+        "cfg2_sin6d_depth1": W.config2(depth=1, budget=0),
+        # BASELINE.json configs[2], whole
+        "cfg3_gauss9d": W.config3(),
+        # BASELINE.json configs[3] with budget 4 per instance (unbudgeted: ~1.7e12 evals)
+        "cfg4_batched4d_B4": W.config4().with_(max_groups_per_level=4),
+        # BASELINE.json configs[4], level 1 only (the 5.2e11 evaluations BASELINE.json quotes)
+        "cfg5_sin6d_level1": W.config5(depth=1),
+        "cfg1_sin3d_f64": W.config1(),
+    }
+
+
+def calls_per_eval(dim):
+    return dim / 4.0     # flat word stream (R3): D words of 32 bits per sample, 4 words per Philox call
+
+
+def alu_peak_evals_per_s(dim, n_sm, sm_mhz):
+    """IMAD.WIDE-pipe roof: one warp-wide IMAD.WIDE.U32 per SM per clock (measured), 20 per Philox call."""
+    clk_per_warp_eval = PHILOX_IMAD_WIDE_PER_CALL * IMAD_WIDE_CLK_PER_WARP_INST_PER_SM * calls_per_eval(dim)
+    return n_sm * sm_mhz * 1e6 * 32.0 / clk_per_warp_eval
+
+
+def launches_per_step(depth):
+    return 2 + 6 * depth + 1     # keys, init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.FIELDS,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            busy = sm[len(sm) // 2:]        # the upper half: samples taken under load
+            out = {"sm_mhz": busy[len(busy) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                   "power_w_max": max(power), "samples": len(sm)}
+        return out
+
+
+def aggregate(ms_local, evals_local, world_size):
+    """max over ranks of the device time, sum over ranks of the evaluations (torch.distributed if N > 1)."""
+    if world_size == 1:
+        return ms_local, evals_local
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms_local], dtype=torch.float64, device=dev)
+    e = torch.tensor([float(evals_local)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(e, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(e.item())
+
+
+def oracle_sample(w, n_units, seed_offset=0):
+    """Time the oracle, as it stands, on n_units (cell, trial) units of level 1 of workload w (single thread).
+    Returns (evals, seconds)."""
+    import numpy as np
+    import oracle as O
+    from tests import helpers as H
+    cfg = H.oracle_config(w)
+    rng = np.random.default_rng(1234 + seed_offset)
+    cells = rng.integers(0, w.k, size=n_units)
+    t0 = time.perf_counter()
+    for i, c in enumerate(cells):
+        path, coords = O.path_coords(w.dim, w.g, [int(c)])
+        O.unit_sum(cfg, int(i % w.n_instances), path, 1, coords, int(i % w.trials))
+    dt = time.perf_counter() - t0
+    return n_units * w.n_samples, dt
+
+
+def run_reference(args, w, name):
+    """--impl reference: the oracle on the host cores, same metric/config; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    units = max(1, int(2.0e7 // w.n_samples))        # ~1 s of single-thread work per step
+    for i in range(args.warmup):
+        oracle_sample(w, max(1, units // 10), i)
+    ev, sec = 0, 0.0
+    for i in range(args.steps):
+        e, s = oracle_sample(w, units, 100 + i)
+        ev += e
+        sec += s
+    val = ev / sec
+    sample = "%d (cell,trial) units of level 1 per step, %d samples each, oracle.unit_sum, single thread" % (units, w.n_samples)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if w.precision == "f32" else "f64", "data": "synthetic",
+            "config": {"workload": name, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2_sin6d_depth3_B16")
+    ap.add_argument("--math", default="exact", choices=["exact", "fast"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    wl = workloads()
+    w = wl[args.workload]
+
+    if args.impl == "reference":
+        run_reference(args, w, args.workload)
+        return
+
+    import numpy as np
+    import torch
+    from paper_1902_07916_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    math = B.MATH_EXACT if args.math == "exact" else B.MATH_FAST
+    w_rank = w.with_(seed=w.seed + rank)            # replicas differ only in the seed
+    cap = 0
+    if w.max_groups_per_level:
+        cap = max(w.k * w.n_instances, w.k * w.n_instances * w.max_groups_per_level)
+    elif w.depth == 1:
+        cap = w.k * w.n_instances
+    it = B.from_workload(w_rank, math=math, max_cells_per_level=cap)
+    it.use_torch_workspace()
+    props = torch.cuda.get_device_properties(local_rank)
+    n_sm = props.multi_processor_count
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        flush.zero_()
+        it.run(stream.cuda_stream)
+    it.result()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_wall = time.perf_counter()
+    e0.record(stream)
+    for _ in range(args.steps):
+        flush.zero_()
+        it.run(stream.cuda_stream)
+    e1.record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    ms_local = e0.elapsed_time(e1)
+    value_v, value_s = it.result()
+    st = it.stats()
+    clocks = sampler.stop() if sampler else None
+    evals_step = int(st.total_evals)
+    ms_total, evals_total = aggregate(ms_local, evals_step * args.steps, world)
+    ms_per_step = ms_total / args.steps
+    value = evals_total / (ms_total * 1e-3)
+
+    # dominant kernel: the fused sampling kernel, timed by the CUDA events zmc_run records around it on its stream
+    samp_ms = sum(st.level[l].sample_ms for l in range(st.levels) if st.level[l].n_cells)
+    ctl_ms = sum(st.level[l].control_ms for l in range(st.levels) if st.level[l].n_cells)
+    n_sample_launches = sum(1 for l in range(st.levels) if st.level[l].n_cells)
+    achieved = evals_step / (samp_ms * 1e-3)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak = alu_peak_evals_per_s(w.dim, n_sm, sm_max)
+    traffic = None
+    tfile = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tfile):
+        traffic = json.load(open(tfile)).get(args.workload)
+    roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s", "frac": achieved / peak,
+                "traffic": traffic,
+                "kernel": "zmc_sample_kernel", "launches_per_step": n_sample_launches, "avg_launch_ms": samp_ms / max(1, n_sample_launches),
+                "share_of_step": samp_ms / (st.total_ms if st.total_ms > 0 else ms_per_step),
+                "peak_basis": "IMAD.WIDE.U32 pipe: %d SMs x %.0f MHz (sm_max_mhz, %s) x 32 lanes / (20 IMAD.WIDE per Philox call x %.2f calls per eval x 1 clk)" %
+                              (n_sm, sm_max, "MEASURED_PEAKS.json" if peaks else "guide nominal", calls_per_eval(w.dim)),
+                "control_ms_per_step": ctl_ms}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if w.precision == "f32" else "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "note": w.note, "dim": w.dim, "divisions_per_axis": w.g, "samples_per_cell": w.n_samples,
+                       "trials": w.trials, "depth": w.depth, "sigma_multiplier": w.sigma_multiplier, "seed": w.seed,
+                       "n_instances": w.n_instances, "max_groups_per_level": w.max_groups_per_level, "math": args.math,
+                       "evals_per_step": evals_step, "l2": "256 MiB buffer written between steps (flush); the path reads ~16 B per cell",
+                       "parallelism": "replicas x%d" % world},
+            "result": {"value": float(value_v[0]), "std": float(value_s[0])},
+            "wall_ms_per_step": 1e3 * t_wall / args.steps,
+            "gpu_launches": launches_per_step(w.depth) * args.steps,
+            "roofline": roofline}
+    if clocks is not None:
+        line["clocks"] = clocks
+
+    if rank == 0:
+        # ---- e2e: the call a user makes, from host arrays to host result, every step
+        e2e_steps = max(1, min(args.steps, 3))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ev = 0
+        for i in range(e2e_steps):
+            it2 = B.from_workload(w_rank, math=math, max_cells_per_level=cap)   # host bounds + params -> zmc_create / zmc_set_integrand
+            it2.use_torch_workspace()
+            it2.run(stream.cuda_stream)                                         # parameters H2D + every kernel
+            it2.result()                                                         # D2H of (value, std) per instance + overflow flag
+            ev += evals_step
+            it2.close()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        npar = 0 if w.params is None else int(np.asarray(w.params).size)
+        line["e2e"] = {"value": ev / dt, "unit": UNIT, "h2d_bytes_per_step": 16 * w.dim + 12 * npar,
+                       "d2h_bytes_per_step": 16 * w.n_instances + 4, "ms_per_step": 1e3 * dt / e2e_steps,
+                       "what": "zmc_create + zmc_set_integrand + zmc_set_option + zmc_set_workspace + zmc_run + zmc_result + zmc_destroy per step, host arrays in, host doubles out"}
+
+        if world == 1 and not args.no_extra and args.workload != "cfg3_gauss9d":
+            # time-to-result of the 9-D workload (BASELINE.json metric: "time-to-result at 6-D and 9-D")
+            w3 = wl["cfg3_gauss9d"]
+            it3 = B.from_workload(w3, math=math, max_cells_per_level=2 * w3.k)
+            for _ in range(3):
+                it3.run(stream.cuda_stream)
+            v3, s3 = it3.result()
+            st3 = it3.stats()
+            line["time_to_result"] = {args.workload: {"ms": ms_per_step, "value": float(value_v[0]), "std": float(value_s[0])},
+                                      "cfg3_gauss9d": {"ms": st3.total_ms, "value": float(v3[0]), "std": float(s3[0]),
+                                                       "evals": int(st3.total_evals),
+                                                       "evals_per_s": st3.total_evals / (st3.total_ms * 1e-3)}}
+            it3.close()
+
+        if world == 1 and not args.no_cpu_baseline:
+            units = max(1, int(2.0e8 // w.n_samples))
+            ev_c, sec_c = oracle_sample(w, units)
+            line["cpu_baseline"] = {"value": ev_c / sec_c, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": "%d (cell,trial) units of level 1 of %s, %d samples each, single thread, %.1f s" %
+                                              (units, args.workload, w.n_samples, sec_c)}
+        print(json.dumps(line), flush=True)
+    it.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
