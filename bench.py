@@ -59,6 +59,21 @@ def alu_peak_evals_per_s(dim, n_sm, sm_mhz):
     return n_sm * sm_mhz * 1e6 * 32.0 / clk_per_warp_eval
 
 
+def traffic_from_profiles(workload, math):
+    """DRAM bytes (read + write) per launch of the sampling kernel from the committed ncu --set full summary
+    (profiles/traffic.csv): the mean over the launches captured for this workload, or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    vals = []
+    for line in open(path):
+        parts = [x.strip() for x in line.split(",")]
+        if line.startswith("#") or len(parts) < 5 or parts[0] != workload or parts[1] != math:
+            continue
+        vals.append(float(parts[3]) + float(parts[4]))
+    return sum(vals) / len(vals) if vals else None
+
+
 def launches_per_step(depth):
     return 2 + 6 * depth + 1     # keys, init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
 
@@ -255,10 +270,7 @@ def main():
         pass
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = alu_peak_evals_per_s(w.dim, n_sm, sm_max)
-    traffic = None
-    tfile = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tfile):
-        traffic = json.load(open(tfile)).get(args.workload)
+    traffic = traffic_from_profiles(args.workload, args.math)
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s", "frac": achieved / peak,
                 "traffic": traffic,
                 "kernel": "zmc_sample_kernel", "launches_per_step": n_sample_launches, "avg_launch_ms": samp_ms / max(1, n_sample_launches),
