@@ -46,7 +46,21 @@ def workloads():
         # BASELINE.json configs[4], level 1 only (the 5.2e11 evaluations BASELINE.json quotes)
         "cfg5_sin6d_level1": W.config5(depth=1),
         "cfg1_sin3d_f64": W.config1(),
+        # the paper's 12-D Gaussian (Table 4: 47.6 s on one V100), paper's own sizes
+        "cfg12_gauss12d": W.gauss12d(),
     }
+
+
+def capacity_for(w):
+    """max_cells_per_level the bench (and the full-size parity tests) run a workload with: what its budget
+    or depth bounds, else 0 = the library's automatic capacity."""
+    if w.max_cells_per_level:
+        return w.max_cells_per_level
+    if w.max_groups_per_level:
+        return w.k * w.n_instances * max(1, w.max_groups_per_level)
+    if w.depth == 1:
+        return w.k * w.n_instances
+    return 0
 
 
 def calls_per_eval(dim):
@@ -216,11 +230,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     math = B.MATH_EXACT if args.math == "exact" else B.MATH_FAST
     w_rank = w.with_(seed=w.seed + rank)            # replicas differ only in the seed
-    cap = 0
-    if w.max_groups_per_level:
-        cap = max(w.k * w.n_instances, w.k * w.n_instances * w.max_groups_per_level)
-    elif w.depth == 1:
-        cap = w.k * w.n_instances
+    cap = capacity_for(w)
     it = B.from_workload(w_rank, math=math, max_cells_per_level=cap)
     it.use_torch_workspace()
     props = torch.cuda.get_device_properties(local_rank)
@@ -317,7 +327,7 @@ def main():
         if world == 1 and not args.no_extra and args.workload != "cfg3_gauss9d":
             # time-to-result of the 9-D workload (BASELINE.json metric: "time-to-result at 6-D and 9-D")
             w3 = wl["cfg3_gauss9d"]
-            it3 = B.from_workload(w3, math=math, max_cells_per_level=2 * w3.k)
+            it3 = B.from_workload(w3, math=math, max_cells_per_level=capacity_for(w3))
             for _ in range(3):
                 it3.run(stream.cuda_stream)
             v3, s3 = it3.result()

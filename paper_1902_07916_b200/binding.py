@@ -251,8 +251,8 @@ def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool 
         it.set_option(OPT_MAX_GROUPS_PER_LEVEL, w.max_groups_per_level)
     if keep_level_stats:
         it.set_option(OPT_KEEP_LEVEL_STATS, 1)
-    if max_cells_per_level:
-        it.set_option(OPT_MAX_CELLS_PER_LEVEL, max_cells_per_level)
+    if max_cells_per_level or w.max_cells_per_level:
+        it.set_option(OPT_MAX_CELLS_PER_LEVEL, max_cells_per_level or w.max_cells_per_level)
     return it
 
 

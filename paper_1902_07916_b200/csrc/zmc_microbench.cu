@@ -77,6 +77,18 @@ __global__ void __launch_bounds__(256, 4) mb_kernel(zu32* sink, unsigned long lo
                 asm volatile("" : "+r"(r[i]));
             } else if (WHICH == 12) {    /* LEA.HI-like: (w >> 9) | 0x3F800000 */
                 asm volatile("{ .reg .b32 t; shr.u32 t, %0, 9; or.b32 %0, t, 0x3F800000; }" : "+r"(r[i]));
+            } else if (WHICH == 13) {    /* IMAD (low 32 bits of a 32x32 product, plus an addend) */
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k0), "r"(k1));
+            } else if (WHICH == 14) {    /* IMAD.HI.U32 */
+                asm volatile("mul.hi.u32 %0, %0, %1;" : "+r"(r[i]) : "r"(k0));
+            } else if (WHICH == 15) {    /* 64-bit add: IADD3 + IADD3.X (counted as one) */
+                asm volatile("{ add.cc.u32 %0, %0, %2; addc.u32 %1, %1, %3; }"
+                             : "+r"(r[i]), "+r"(r[(i + 1) % kIlp]) : "r"(k0), "r"(k1));
+            } else if (WHICH == 16) {    /* IMAD.WIDE.U32 with a register (not immediate) multiplier */
+                zu32 lo, hi;
+                asm volatile("{ .reg .b64 t; mul.wide.u32 t, %2, %3; mov.b64 {%0,%1}, t; }" : "=r"(lo), "=r"(hi) : "r"(r[i]), "r"(k0));
+                r[i] = hi ^ 0u;
+                (void)lo;
             }
         }
         if (WHICH == 10) {               /* whole Philox4x32-10 calls, kIlp/2 independent calls per step */
@@ -137,6 +149,10 @@ extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, doubl
             case 10: e = launch<10>(grid, sink, cyc, st); break;
             case 11: e = launch<11>(grid, sink, cyc, st); break;
             case 12: e = launch<12>(grid, sink, cyc, st); break;
+            case 13: e = launch<13>(grid, sink, cyc, st); break;
+            case 14: e = launch<14>(grid, sink, cyc, st); break;
+            case 15: e = launch<15>(grid, sink, cyc, st); break;
+            case 16: e = launch<16>(grid, sink, cyc, st); break;
             default: e = cudaErrorInvalidValue;
         }
         cudaEventRecord(e1, st);
@@ -148,7 +164,7 @@ extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, doubl
     cudaEventDestroy(e1);
     cudaFree(sink);
     cudaFree(cyc);
-    if (e != cudaSuccess) return which < 0 || which > 12 ? ZMC_ERR_ARG : ZMC_ERR_CUDA;
+    if (e != cudaSuccess) return which < 0 || which > 16 ? ZMC_ERR_ARG : ZMC_ERR_CUDA;
     /* per thread: kIters * kIlp instructions (which 2: 2 each ; which 10: kIlp/2 Philox calls per step) */
     double per_thread = (double)kIters * kIlp;
     if (which == 2) per_thread *= 2.0;

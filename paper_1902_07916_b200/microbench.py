@@ -1,0 +1,29 @@
+"""Issue-rate microbenchmarks of the pipes the sampling kernel uses (zmc_microbench in include/zmc.h).
+
+    python -m paper_1902_07916_b200.microbench            # prints a markdown table (needs a B200)
+
+They give the denominator of the ALU roofline: warp-instructions per SM per clock
+for IMAD.WIDE.U32, LOP3, FFMA, ... and whole Philox4x32-10 calls.
+"""
+from . import binding as B
+
+NAMES = {0: "IMAD.WIDE.U32", 1: "LOP3", 2: "IMAD.WIDE.U32 + LOP3 (Philox round mix)", 3: "FFMA", 4: "FADD", 5: "DADD",
+         6: "F2F.F64.F32", 7: "MUFU.SIN", 8: "MUFU.EX2", 9: "DFMA", 10: "Philox4x32-10 calls (x32 lanes)",
+         11: "I2F.F64.U32", 12: "LEA.HI-like (shr + or)", 13: "IMAD.U32 lo", 14: "IMAD.HI.U32",
+         15: "IADD3 + IADD3.X (64-bit add)", 16: "IMAD.WIDE.U32 with register multiplier"}
+
+
+def main():
+    print("| which | instruction | warp-instr / SM / clk | clocks per warp-instr per sub-partition | SM MHz |")
+    print("|---|---|---|---|---|")
+    for w in sorted(NAMES):
+        try:
+            r, mhz = B.microbench(w)
+        except B.ZmcError as e:
+            print("| %d | %s | error %d | | |" % (w, NAMES[w], e.status))
+            continue
+        print("| %d | %s | %.3f | %.2f | %.0f |" % (w, NAMES[w], r, 4.0 / r if r > 0 else float("nan"), mhz))
+
+
+if __name__ == "__main__":
+    main()

@@ -35,6 +35,7 @@ class Workload:
     params: Optional[np.ndarray] = None   # [n_instances, params_per_instance], float64
     n_instances: int = 1
     max_groups_per_level: int = 0         # R12 refinement budget (0 = off = paper semantics)
+    max_cells_per_level: int = 0          # capacity hint for one level (0 = library default); exceeding it is an error
     note: str = ""
 
     @property
@@ -79,7 +80,8 @@ def config2(depth: int = 3, budget: int = 0) -> Workload:
 
 def config3() -> Workload:
     return Workload("cfg3_gauss9d", 9, (-1.0,) * 9, (1.0,) * 9, 3, 20000, 5, 4, 1.0, 3, EXP_QUAD, F32,
-                    params=gaussian_params(9, 0.01), note="BASELINE.json configs[2]; paper f2, Eq. (2)")
+                    params=gaussian_params(9, 0.01), max_cells_per_level=4 * 3 ** 9,
+                    note="BASELINE.json configs[2]; paper f2, Eq. (2)")
 
 
 def config4(n_instances: int = 1024) -> Workload:
@@ -92,3 +94,11 @@ def config4(n_instances: int = 1024) -> Workload:
 def config5(depth: int = 4, budget: int = 0) -> Workload:
     return Workload("cfg5_sin6d_stress", 6, (0.0,) * 6, (10.0,) * 6, 8, 200000, 10, depth, 1.0, 5, SIN_SUM, F32,
                     max_groups_per_level=budget, note="BASELINE.json configs[4]")
+
+
+def gauss12d() -> Workload:
+    """the 12-D Gaussian of the paper's Table 4 at the paper's own sizes:
+    3 divisions per axis (531441 cells), 1e4 samples per cell, 5 trials, depth 4, "4 sigma" threshold."""
+    return Workload("cfg12_gauss12d", 12, (-1.0,) * 12, (1.0,) * 12, 3, 10000, 5, 4, 4.0, 12, EXP_QUAD, F32,
+                    params=gaussian_params(12, 0.01), max_cells_per_level=4 * 3 ** 12,
+                    note="paper Table 4 (PAPER.md:202-216); f2, Eq. (2), D = 12")
