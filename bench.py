@@ -89,7 +89,8 @@ def traffic_from_profiles(workload, math):
 
 
 def launches_per_step(depth):
-    return 2 + 6 * depth + 1     # keys, init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
+    return 1 + 6 * depth + 1     # init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
+                                 # (zmc_keys_kernel runs once per context, with the parameter upload)
 
 
 class ClockSampler:

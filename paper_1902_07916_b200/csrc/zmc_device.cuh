@@ -25,9 +25,6 @@ typedef int zi32;
 #ifndef ZMC_BLOCK_THREADS
 #define ZMC_BLOCK_THREADS 128
 #endif
-#ifndef ZMC_MIN_BLOCKS
-#define ZMC_MIN_BLOCKS 4
-#endif
 
 /* integrand ids / precision / math mode: values mirror include/zmc.h (checked by static_assert in zmc_lib.cu) */
 #define ZMC_ID_CONST 0
@@ -70,6 +67,7 @@ struct ZmcSampleArgs {
     zu64 N;
     double lower[ZMC_DEV_MAX_DIM];
     double width[ZMC_DEV_MAX_DIM];   /* cell width at this level, (upper-lower)/g^level (R2) */
+    zu32 ukey[2];                    /* UKEY kernels (n_instances == 1): the one derived key, read from the constant bank */
 };
 
 /* ------------------------------------------------------------------ R1: Philox4x32-10 */
@@ -134,7 +132,8 @@ __device__ __forceinline__ float zmc_zsin(float a) {
     p = __fmaf_rn(p, s, C3);
     const float rs = __fmul_rn(r, s);
     const float v = __fmaf_rn(rs, p, r);
-    return __uint_as_float(__float_as_uint(v) ^ (__float_as_uint(t) << 31));
+    /* sign (-1)^k: bit 0 of t into bit 31 of v. v + (t << 31) mod 2^32 = v ^ ((t & 1) << 31): one IMAD */
+    return __uint_as_float(__float_as_uint(t) * 0x80000000u + __float_as_uint(v));
 }
 
 /* zexp: n = rint(e*log2 e) by the magic-number add, two-constant reduction r = e - n ln2, degree-6
@@ -163,9 +162,10 @@ __device__ __forceinline__ double zmc_zexp_value(float e) {
     p = __fmaf_rn(p, r, E2);
     p = __fmaf_rn(p, r, 1.0f);
     p = __fmaf_rn(p, r, 1.0f);
-    const zi32 n = (zi32)(__float_as_uint(t) - 0x4b400000u);
+    /* n = bits(t) - 0x4b400000; only the low 12 bits of n survive "<< 20" and 0x4b400000 has none set,
+     * so bits(t) << 20 is n << 20 */
     const double dp = (double)p;
-    return __hiloint2double(__double2hiint(dp) + (n << 20), __double2loint(dp));
+    return __hiloint2double(__double2hiint(dp) + (zi32)(__float_as_uint(t) << 20), __double2loint(dp));
 }
 
 /* fast mode: the same split e*log2e = n + r, with 2^r from MUFU.EX2 */
@@ -187,6 +187,74 @@ __device__ __forceinline__ double zmc_fexp_value(float e) {
     return __hiloint2double(__double2hiint(dp) + (n << 20), __double2loint(dp));
 }
 
+
+/* ------------------------------------------------------------------ packed FP32 pairs (FFMA2 / FADD2 / FMUL2, new on sm_100) */
+/* Two samples share one instruction: fma/add/mul.rn.f32x2 are component-wise IEEE round-to-nearest,
+ * so a packed sequence gives bit for bit what the scalar sequence gives on each component (R8).
+ * A broadcast operand (v, v) costs no register: ptxas encodes it as a scalar/immediate operand.
+ * Why it pays: the path is bound by dispatch slots, and one FFMA2 costs less
+ * than two FFMA there. */
+typedef unsigned long long zf2;
+__device__ __forceinline__ zf2 zmc_pk(float lo, float hi) { zf2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ zf2 zmc_bc(float v) { return zmc_pk(v, v); }
+__device__ __forceinline__ float zmc_lo(zf2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)b; return a; }
+__device__ __forceinline__ float zmc_hi(zf2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)a; return b; }
+__device__ __forceinline__ zf2 zmc_fma2(zf2 a, zf2 b, zf2 c) { zf2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ zf2 zmc_add2(zf2 a, zf2 b) { zf2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ zf2 zmc_mul2(zf2 a, zf2 b) { zf2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
+/* zmc_zsin on a pair: the same operation sequence, component-wise */
+__device__ __forceinline__ zf2 zmc_zsin2(zf2 a) {
+    const float INV_PI = __uint_as_float(0x3ea2f983u);
+    const float MAGIC = __uint_as_float(0x4b400000u);
+    const float NPI_A = __uint_as_float(0xc0490000u);
+    const float NPI_B = __uint_as_float(0xba7daa22u);
+    const float C3 = __uint_as_float(0xbe2aaaa6u), C5 = __uint_as_float(0x3c08876au);
+    const float C7 = __uint_as_float(0xb94fb7f7u), C9 = __uint_as_float(0x362ede75u);
+    const zf2 t = zmc_fma2(a, zmc_bc(INV_PI), zmc_bc(MAGIC));
+    const zf2 kf = zmc_add2(t, zmc_bc(-MAGIC));
+    zf2 r = zmc_fma2(kf, zmc_bc(NPI_A), a);
+    r = zmc_fma2(kf, zmc_bc(NPI_B), r);
+    const zf2 s = zmc_mul2(r, r);
+    zf2 p = zmc_fma2(zmc_bc(C9), s, zmc_bc(C7));
+    p = zmc_fma2(p, s, zmc_bc(C5));
+    p = zmc_fma2(p, s, zmc_bc(C3));
+    const zf2 rs = zmc_mul2(r, s);
+    const zf2 v = zmc_fma2(rs, p, r);
+    const zu32 vl = __float_as_uint(zmc_lo(t)) * 0x80000000u + __float_as_uint(zmc_lo(v));
+    const zu32 vh = __float_as_uint(zmc_hi(t)) * 0x80000000u + __float_as_uint(zmc_hi(v));
+    return zmc_pk(__uint_as_float(vl), __uint_as_float(vh));
+}
+
+/* zmc_zexp_value on a pair: packed reduction and polynomial, then each component assembled as there */
+__device__ __forceinline__ double zmc_zexp_finish(float e, float t, float p) {
+    const double dp = (double)p;
+    double v = __hiloint2double(__double2hiint(dp) + (zi32)(__float_as_uint(t) << 20), __double2loint(dp));
+    if (!(fabsf(e) <= 708.0f))
+        v = (e < 0.0f) ? 0.0 : ((e > 0.0f) ? __longlong_as_double(0x7FF0000000000000ll) : __longlong_as_double(0x7FF8000000000000ll));
+    return v;
+}
+__device__ __forceinline__ void zmc_zexp2(zf2 e, double& fa, double& fb) {
+    const float LOG2E = __uint_as_float(0x3fb8aa3bu);
+    const float MAGIC = __uint_as_float(0x4b400000u);
+    const float NLN2_HI = __uint_as_float(0xbf317200u);
+    const float NLN2_LO = __uint_as_float(0xb5bfbe8eu);
+    const float E2 = __uint_as_float(0x3efffffeu), E3 = __uint_as_float(0x3e2aaa49u), E4 = __uint_as_float(0x3d2aac79u);
+    const float E5 = __uint_as_float(0x3c091cf1u), E6 = __uint_as_float(0x3ab5121au);
+    const zf2 t = zmc_fma2(e, zmc_bc(LOG2E), zmc_bc(MAGIC));
+    const zf2 nf = zmc_add2(t, zmc_bc(-MAGIC));
+    zf2 r = zmc_fma2(nf, zmc_bc(NLN2_HI), e);
+    r = zmc_fma2(nf, zmc_bc(NLN2_LO), r);
+    zf2 p = zmc_fma2(zmc_bc(E6), r, zmc_bc(E5));
+    p = zmc_fma2(p, r, zmc_bc(E4));
+    p = zmc_fma2(p, r, zmc_bc(E3));
+    p = zmc_fma2(p, r, zmc_bc(E2));
+    p = zmc_fma2(p, r, zmc_bc(1.0f));
+    p = zmc_fma2(p, r, zmc_bc(1.0f));
+    fa = zmc_zexp_finish(zmc_lo(e), zmc_lo(t), zmc_lo(p));
+    fb = zmc_zexp_finish(zmc_hi(e), zmc_hi(t), zmc_hi(p));
+}
+
 /* ------------------------------------------------------------------ R2 + R4: cell geometry and the word -> point map */
 /* lo_d = lower_d + (double)I_d * width_d (multiply, then add).
  * FP64: x = lo + ((double)w + 0.5) * (width * 2^-32).
@@ -204,6 +272,10 @@ struct ZmcMapF32 {
     }
     __device__ __forceinline__ float x(int d, zu32 w) const {
         return __fmaf_rn(__uint_as_float(0x3F800000u | (w >> 9)), wf[d], base[d]);
+    }
+    __device__ __forceinline__ zf2 x2(int d, zu32 wa, zu32 wb) const {   /* two samples' coordinate d */
+        return zmc_fma2(zmc_pk(__uint_as_float(0x3F800000u | (wa >> 9)), __uint_as_float(0x3F800000u | (wb >> 9))),
+                        zmc_bc(wf[d]), zmc_bc(base[d]));
     }
 };
 
@@ -294,6 +366,48 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
 #endif
         return 0.0;
     }
+
+    /* Two samples at once on the packed FP32 instructions: component-wise the operation sequence of eval(),
+     * hence the same bits (checked by the P1 parity test through zmc_points_kernel). */
+    static constexpr bool HAS_PACKED = (ID == ZMC_ID_SIN_SUM || ID == ZMC_ID_EXP_QUAD || ID == ZMC_ID_LINEAR);
+    __device__ __forceinline__ void eval2(const zu32* wa, const zu32* wb, double& fa, double& fb) const {
+        if (!HAS_PACKED) { fa = eval(wa, nullptr); fb = eval(wb, nullptr); return; }
+        zf2 x[D_];
+#pragma unroll
+        for (int d = 0; d < D_; ++d) x[d] = map.x2(d, wa[d], wb[d]);
+        if (ID == ZMC_ID_LINEAR) {
+            zf2 f = zmc_bc(c0);
+#pragma unroll
+            for (int d = 0; d < D_; ++d) f = zmc_fma2(zmc_bc(lin[d]), x[d], f);
+            fa = (double)zmc_lo(f);
+            fb = (double)zmc_hi(f);
+        }
+        if (ID == ZMC_ID_SIN_SUM) {
+            zf2 s = x[0];
+#pragma unroll
+            for (int d = 1; d < D_; ++d) s = zmc_add2(s, x[d]);
+            if (MODE == ZMC_MODE_FAST) {
+                fa = (double)__sinf(zmc_lo(s));
+                fb = (double)__sinf(zmc_hi(s));
+            } else {
+                const zf2 v = zmc_zsin2(s);
+                fa = (double)zmc_lo(v);
+                fb = (double)zmc_hi(v);
+            }
+        }
+        if (ID == ZMC_ID_EXP_QUAD) {
+            zf2 q = zmc_mul2(x[0], x[0]);
+#pragma unroll
+            for (int d = 1; d < D_; ++d) q = zmc_fma2(x[d], x[d], q);
+            const zf2 e = zmc_mul2(zmc_bc(c0), q);
+            if (MODE == ZMC_MODE_FAST) {
+                fa = zmc_fexp_value(zmc_lo(e));
+                fb = zmc_fexp_value(zmc_hi(e));
+            } else {
+                zmc_zexp2(e, fa, fb);
+            }
+        }
+    }
 };
 
 template <int ID, int D_, int MODE>
@@ -360,6 +474,11 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
 #endif
         return 0.0;
     }
+    static constexpr bool HAS_PACKED = false;   /* there is no packed FP64 */
+    __device__ __forceinline__ void eval2(const zu32* wa, const zu32* wb, double& fa, double& fb) const {
+        fa = eval(wa, nullptr);
+        fb = eval(wb, nullptr);
+    }
 };
 
 /* ------------------------------------------------------------------ work-item decoding (R2) */
@@ -405,6 +524,19 @@ template <int D> struct ZmcGroup {
     static constexpr int CG = D / G4;
 };
 
+/* Per-instance tuning of the sampling kernel (measured on B200; profiles/r1_variants.md). The path is
+ * bound by dispatch slots, so what is tuned is the instruction count and the compiler's schedule:
+ *   PACKED  evaluate two samples per FFMA2/FADD2/FMUL2 (needs F::HAS_PACKED)
+ *   UNROLL  sample groups in flight per lane and loop trip: 2 or 4
+ *   MINB    resident CTAs per SM asked of __launch_bounds__ (register cap) */
+template <class F>
+struct ZmcTune {
+    static constexpr int D = F::D;
+    static constexpr bool PACKED = F::HAS_PACKED && ((D == 4) || (D == 6) || (D % 2 == 0 && D <= 8));
+    static constexpr int UNROLL = (D == 4 || D == 6 || D == 12) ? 4 : 2;
+    static constexpr int MINB = (D == 4) ? 4 : 3;
+};
+
 template <class F>
 __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
                                                double* acc) {
@@ -413,12 +545,46 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
     const zu32 q0 = gi * (zu32)CG;
 #pragma unroll
     for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+    if (ZmcTune<F>::PACKED && SG >= 2) {      /* samples (2i, 2i+1) of the group as one packed evaluation */
 #pragma unroll
-    for (int s = 0; s < SG; ++s) acc[s] = __dadd_rn(acc[s], f.eval(&w[s * D], nullptr));
+        for (int s = 0; s < SG; s += 2) {
+            double fa, fb;
+            f.eval2(&w[s * D], &w[(s + 1) * D], fa, fb);
+            acc[s] = __dadd_rn(acc[s], fa);
+            acc[s + 1] = __dadd_rn(acc[s + 1], fb);
+        }
+    } else {
+#pragma unroll
+        for (int s = 0; s < SG; ++s) acc[s] = __dadd_rn(acc[s], f.eval(&w[s * D], nullptr));
+    }
 }
 
+/* groups gi and gj: acc[0..SG) takes gi's samples, acc[SG..2SG) gj's -- the same sums as two zmc_group_eval calls */
 template <class F>
-__global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZMC_MIN_BLOCKS) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
+__device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
+                                                    zu32 gj, double* acc) {
+    constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
+    if (ZmcTune<F>::PACKED && SG == 1) {      /* one sample per group (D = 4, 8, ..): pack across the two groups */
+        zu32 wa[4 * CG], wb[4 * CG];
+#pragma unroll
+        for (int c = 0; c < CG; ++c) zmc_philox(gi * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wa[4 * c]);
+#pragma unroll
+        for (int c = 0; c < CG; ++c) zmc_philox(gj * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wb[4 * c]);
+        double fa, fb;
+        f.eval2(wa, wb, fa, fb);
+        acc[0] = __dadd_rn(acc[0], fa);
+        acc[1] = __dadd_rn(acc[1], fb);
+    } else {
+        zmc_group_eval(f, ks, uc, gi, acc);
+        zmc_group_eval(f, ks, uc, gj, acc + SG);
+    }
+}
+
+/* UKEY: every work item has the same Philox key (n_instances == 1); it comes from the kernel
+ * parameters (constant bank), so the ten round keys live in uniform registers: 20 fewer registers
+ * per thread and one register operand fewer on every Philox LOP3. */
+template <class F, bool UKEY>
+__global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     const zu32 lane = threadIdx.x & 31u;
     ZmcLevelInfo* const info = a.info;
@@ -440,7 +606,8 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZMC_MIN_BLOCKS) zmc_sample_
         F f;
         f.setup(a, u.inst, u.coords);
         ZmcKeySchedule ks;
-        ks.init(a.keys[2 * u.inst], a.keys[2 * u.inst + 1]);
+        if (UKEY) ks.init(a.ukey[0], a.ukey[1]);
+        else ks.init(a.keys[2 * u.inst], a.keys[2 * u.inst + 1]);
         ZmcUnitCounter uc;
         uc.init(u.path_lo, u.path_hi, a.level, u.trial);
 
@@ -448,14 +615,19 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZMC_MIN_BLOCKS) zmc_sample_
         const zu32 ge = (gb + chunk_groups < n_groups) ? gb + chunk_groups : n_groups;
         const zu32 gfe = (ge < full_groups) ? ge : full_groups;
 
+        /* lanes stride over the chunk's groups; acc[0..SG) sums the groups at even multiples of 32 from the
+         * lane's first one, acc[SG..2SG) those at odd multiples -- whatever UNROLL is, so results do not depend on it */
         double acc[2 * SG];
 #pragma unroll
         for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
         zu32 gi = gb + lane;
-        for (; gi + 32u < gfe; gi += 64u) {
-            zmc_group_eval(f, ks, uc, gi, acc);
-            zmc_group_eval(f, ks, uc, gi + 32u, acc + SG);
+        if (ZmcTune<F>::UNROLL == 4) {
+            for (; gi + 96u < gfe; gi += 128u) {
+                zmc_group_eval_pair(f, ks, uc, gi, gi + 32u, acc);
+                zmc_group_eval_pair(f, ks, uc, gi + 64u, gi + 96u, acc);
+            }
         }
+        for (; gi + 32u < gfe; gi += 64u) zmc_group_eval_pair(f, ks, uc, gi, gi + 32u, acc);
         if (gi < gfe) zmc_group_eval(f, ks, uc, gi, acc);
         if (tail != 0u && ge > full_groups && lane == 0u) {   /* the partial group: only its first `tail` samples exist */
             zu32 w[4 * CG];
@@ -487,6 +659,21 @@ struct ZmcPointsArgs {
     double* f;              /* [n] */
 };
 
+template <int D>
+__device__ __forceinline__ void zmc_sample_words(zu64 s, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32* w) {
+    zu32 cur[4];
+    zu64 have = ~0ull;
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+        const zu64 idx = s * (zu64)D + (zu64)d;
+        if ((idx >> 2) != have) { have = idx >> 2; zmc_philox((zu32)have, uc.c1, uc.c2, uc.c3, ks, cur); }
+        w[d] = cur[idx & 3ull];
+    }
+}
+
+/* One thread per pair of samples (2t, 2t+1). x always comes from the scalar eval(); f comes from the
+ * packed eval2() for even t and from the scalar eval() for odd t, so a bit-exact comparison of f with
+ * the oracle covers both code paths of the sampling kernel. */
 template <class F>
 __global__ void zmc_points_kernel(const __grid_constant__ ZmcPointsArgs pa) {
     constexpr int D = F::D;
@@ -499,22 +686,25 @@ __global__ void zmc_points_kernel(const __grid_constant__ ZmcPointsArgs pa) {
     ks.init(pa.a.keys[2 * pa.inst], pa.a.keys[2 * pa.inst + 1]);
     ZmcUnitCounter uc;
     uc.init(pa.path_lo, pa.path_hi, pa.a.level, pa.trial);
-    for (zu64 s = (zu64)blockIdx.x * blockDim.x + threadIdx.x; s < pa.n; s += (zu64)gridDim.x * blockDim.x) {
-        zu32 w[D];
-        zu32 cur[4];
-        zu64 have = ~0ull;
-#pragma unroll
-        for (int d = 0; d < D; ++d) {
-            const zu64 idx = s * (zu64)D + (zu64)d;
-            if ((idx >> 2) != have) { have = idx >> 2; zmc_philox((zu32)have, uc.c1, uc.c2, uc.c3, ks, cur); }
-            w[d] = cur[idx & 3ull];
+    const zu64 n_pairs = (pa.n + 1ull) >> 1;
+    for (zu64 t = (zu64)blockIdx.x * blockDim.x + threadIdx.x; t < n_pairs; t += (zu64)gridDim.x * blockDim.x) {
+        const zu64 s0 = 2ull * t, s1 = s0 + 1ull;
+        zu32 w0[D], w1[D];
+        zmc_sample_words<D>(s0, ks, uc, w0);
+        zmc_sample_words<D>(s1, ks, uc, w1);
+        double x0[D], x1[D];
+        double v0 = f.eval(w0, x0), v1 = f.eval(w1, x1);
+        if ((t & 1ull) == 0ull) f.eval2(w0, w1, v0, v1);
+        if (pa.f) {
+            pa.f[s0] = v0;
+            if (s1 < pa.n) pa.f[s1] = v1;
         }
-        double xo[D];
-        const double v = f.eval(w, xo);
-        if (pa.f) pa.f[s] = v;
         if (pa.x) {
 #pragma unroll
-            for (int d = 0; d < D; ++d) pa.x[s * D + d] = xo[d];
+            for (int d = 0; d < D; ++d) {
+                pa.x[s0 * D + d] = x0[d];
+                if (s1 < pa.n) pa.x[s1 * D + d] = x1[d];
+            }
         }
     }
 }

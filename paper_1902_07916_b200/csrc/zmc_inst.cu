@@ -12,7 +12,8 @@ template <int D>
 static ZmcKernelEntry zmc_entry() {
     using F = ZmcIntegrand<ZMC_INST_ID, D, ZMC_INST_PREC, ZMC_INST_MODE>;
     ZmcKernelEntry e;
-    e.sample = (const void*)zmc_sample_kernel<F>;
+    e.sample = (const void*)zmc_sample_kernel<F, false>;
+    e.sample_ukey = (const void*)zmc_sample_kernel<F, true>;
     e.points = (const void*)zmc_points_kernel<F>;
     return e;
 }
@@ -35,6 +36,6 @@ ZmcKernelEntry ZMC_LOOKUP_NAME(ZMC_INST_PREC, ZMC_INST_MODE, ZMC_INST_ID)(int di
         case 11: return zmc_entry<11>();
         case 12: return zmc_entry<12>();
     }
-    ZmcKernelEntry none = {nullptr, nullptr};
+    ZmcKernelEntry none = {nullptr, nullptr, nullptr};
     return none;
 }

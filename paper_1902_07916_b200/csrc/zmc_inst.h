@@ -6,7 +6,8 @@
 #define ZMC_AOT_MAX_DIM 12
 
 struct ZmcKernelEntry {
-    const void* sample;   /* zmc_sample_kernel<F> */
+    const void* sample;       /* zmc_sample_kernel<F, false>: per-item key (batched instances) */
+    const void* sample_ukey;  /* zmc_sample_kernel<F, true>: one key for the whole launch (n_instances == 1) */
     const void* points;   /* zmc_points_kernel<F> */
 };
 

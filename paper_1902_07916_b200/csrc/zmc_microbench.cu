@@ -115,6 +115,94 @@ cudaError_t launch(int grid, zu32* sink, unsigned long long* cyc, cudaStream_t s
     return cudaGetLastError();
 }
 
+/* Philox4x32-10 calls with K extra independent instructions of kind X after each call: the slope of
+ * clocks-per-call against K is what one more instruction of that kind costs next to the generator
+ * (the dispatch-slot model). 4 independent calls per thread, 8 warps per scheduler.
+ * X: 1 LOP3, 2 FFMA, 3 FADD, 4 DADD, 5 FFMA2, 6 IMAD (lo), 7 SHF */
+template <int X, int K>
+__global__ void __launch_bounds__(256, 4) mbx_kernel(zu32* sink, unsigned long long* cycles, zu32 seed) {
+    zu32 r[8];
+    float f[8];
+    zu64 d[8];
+    double x[8];
+    const zu32 k0 = seed * 3u + 1u, k1 = seed * 5u + 7u;
+    const float fc = __uint_as_float(0x3f7ff000u | (seed & 0xFFu)), fd = fc * 0.5f;
+    const zu64 dc = ((zu64)__float_as_uint(fc) << 32) | __float_as_uint(fc), dd = dc ^ 0x0000100000001000ull;
+    const double xc = (double)fc;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        r[i] = seed + threadIdx.x * 977u + i * 131u;
+        f[i] = __uint_as_float(0x3f800000u | (r[i] & 0xFFFFu));
+        d[i] = ((zu64)__float_as_uint(f[i]) << 32) | __float_as_uint(f[i]);
+        x[i] = f[i];
+    }
+    ZmcKeySchedule ks;
+    ks.init(k0, k1);
+    zu32 c[4][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { c[j][0] = r[j]; c[j][1] = r[j + 4]; c[j][2] = k0 + j; c[j][3] = k1 + j; }
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < kIters / 4; ++it) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            zu32 w[4];
+            zmc_philox(c[j][0] + (zu32)it, c[j][1], c[j][2], c[j][3], ks, w);
+            c[j][0] = w[0]; c[j][1] = w[1]; c[j][2] = w[2]; c[j][3] = w[3];
+#pragma unroll
+            for (int e = 0; e < K; ++e) {
+                const int i = e & 7;
+                if (X == 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[i]) : "r"(k0), "r"(k1));
+                if (X == 2) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[i]) : "f"(fc), "f"(fd));
+                if (X == 3) asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(fc));
+                if (X == 4) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(x[i]) : "d"(xc));
+                if (X == 5) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(d[i]) : "l"(dc), "l"(dd));
+                if (X == 6) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k0), "r"(k1));
+                if (X == 7) asm volatile("shf.l.wrap.b32 %0, %0, %1, 9;" : "+r"(r[i]) : "r"(k0));
+            }
+        }
+    }
+    const long long t1 = clock64();
+    zu32 acc = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc ^= r[i] ^ __float_as_uint(f[i]) ^ (zu32)d[i] ^ (zu32)(d[i] >> 32) ^ (zu32)__double2loint(x[i]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc ^= c[j][0] ^ c[j][1] ^ c[j][2] ^ c[j][3];
+    if (acc == 0x12345678u) sink[0] = acc;
+    if (threadIdx.x == 0) atomicMax(cycles, (unsigned long long)(t1 - t0));
+}
+
+template <int X, int K>
+cudaError_t launchx(int grid, zu32* sink, unsigned long long* cyc, cudaStream_t st) {
+    mbx_kernel<X, K><<<grid, 256, 0, st>>>(sink, cyc, 12345u);
+    return cudaGetLastError();
+}
+
+template <int X>
+cudaError_t launchx_k(int kidx, int grid, zu32* sink, unsigned long long* cyc, cudaStream_t st) {
+    switch (kidx) {
+        case 0: return launchx<X, 0>(grid, sink, cyc, st);
+        case 1: return launchx<X, 10>(grid, sink, cyc, st);
+        case 2: return launchx<X, 20>(grid, sink, cyc, st);
+        case 3: return launchx<X, 40>(grid, sink, cyc, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_mix(int which, int grid, zu32* sink, unsigned long long* cyc, cudaStream_t st) {
+    const int X = (which - 100) / 10, kidx = (which - 100) % 10;
+    switch (X) {
+        case 1: return launchx_k<1>(kidx, grid, sink, cyc, st);
+        case 2: return launchx_k<2>(kidx, grid, sink, cyc, st);
+        case 3: return launchx_k<3>(kidx, grid, sink, cyc, st);
+        case 4: return launchx_k<4>(kidx, grid, sink, cyc, st);
+        case 5: return launchx_k<5>(kidx, grid, sink, cyc, st);
+        case 6: return launchx_k<6>(kidx, grid, sink, cyc, st);
+        case 7: return launchx_k<7>(kidx, grid, sink, cyc, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
 }  // namespace
 
 extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, double* sm_mhz) {
@@ -153,7 +241,7 @@ extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, doubl
             case 14: e = launch<14>(grid, sink, cyc, st); break;
             case 15: e = launch<15>(grid, sink, cyc, st); break;
             case 16: e = launch<16>(grid, sink, cyc, st); break;
-            default: e = cudaErrorInvalidValue;
+            default: e = (which >= 100 && which < 180) ? launch_mix(which, grid, sink, cyc, st) : cudaErrorInvalidValue;
         }
         cudaEventRecord(e1, st);
         if (e == cudaSuccess) e = cudaEventSynchronize(e1);
@@ -164,11 +252,12 @@ extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, doubl
     cudaEventDestroy(e1);
     cudaFree(sink);
     cudaFree(cyc);
-    if (e != cudaSuccess) return which < 0 || which > 16 ? ZMC_ERR_ARG : ZMC_ERR_CUDA;
+    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? ZMC_ERR_ARG : ZMC_ERR_CUDA;
     /* per thread: kIters * kIlp instructions (which 2: 2 each ; which 10: kIlp/2 Philox calls per step) */
     double per_thread = (double)kIters * kIlp;
     if (which == 2) per_thread *= 2.0;
     if (which == 10) per_thread = (double)kIters * (kIlp / 2);
+    if (which >= 100) per_thread = (double)(kIters / 4) * 4.0;   /* Philox calls */
     const double warps_per_sm = 4.0 * 256.0 / 32.0;
     /* all CTAs of an SM are resident at once (4 x 256 threads), so the SM's elapsed clocks ~ the longest CTA */
     if (per_sm_clk) *per_sm_clk = per_thread * warps_per_sm / (double)hc;

@@ -25,5 +25,24 @@ def main():
         print("| %d | %s | %.3f | %.2f | %.0f |" % (w, NAMES[w], r, 4.0 / r if r > 0 else float("nan"), mhz))
 
 
+MIX = {1: "LOP3", 2: "FFMA", 3: "FADD", 4: "DADD", 5: "FFMA2", 6: "IMAD (lo)", 7: "SHF"}
+MIX_K = (0, 10, 20, 40)
+
+
+def mix_table():
+    """Clocks per Philox call per sub-partition with K extra instructions of one kind after each call, and the slope
+    = what one more instruction of that kind costs next to the generator (the dispatch-slot model of DESIGN.md 6)."""
+    print()
+    print("| extra instruction | " + " | ".join("K=%d" % k for k in MIX_K) + " | clocks per extra instruction (K=40 vs K=0) |")
+    print("|---|" + "---|" * (len(MIX_K) + 1))
+    for x in sorted(MIX):
+        clk = []
+        for j, k in enumerate(MIX_K):
+            r, _ = B.microbench(100 + 10 * x + j)
+            clk.append(4.0 / r)
+        print("| %s | " % MIX[x] + " | ".join("%.1f" % c for c in clk) + " | %.2f |" % ((clk[-1] - clk[0]) / MIX_K[-1]))
+
+
 if __name__ == "__main__":
     main()
+    mix_table()
