@@ -291,6 +291,13 @@ struct ZmcMapF64 {
     }
 };
 
+#ifndef ZMC_PACKED_SIN_POLY
+#define ZMC_PACKED_SIN_POLY(D) 1
+#endif
+#ifndef ZMC_PACKED_EXP_POLY
+#define ZMC_PACKED_EXP_POLY(D) ((D) <= 8)
+#endif
+
 /* ------------------------------------------------------------------ integrands */
 /* Each integrand policy has
  *   setup(args, instance, coords)  once per work item: geometry and this instance's parameters
@@ -389,10 +396,13 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
             if (MODE == ZMC_MODE_FAST) {
                 fa = (double)__sinf(zmc_lo(s));
                 fb = (double)__sinf(zmc_hi(s));
-            } else {
+            } else if (ZMC_PACKED_SIN_POLY(D_)) {
                 const zf2 v = zmc_zsin2(s);
                 fa = (double)zmc_lo(v);
                 fb = (double)zmc_hi(v);
+            } else {
+                fa = (double)zmc_zsin(zmc_lo(s));
+                fb = (double)zmc_zsin(zmc_hi(s));
             }
         }
         if (ID == ZMC_ID_EXP_QUAD) {
@@ -403,8 +413,11 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
             if (MODE == ZMC_MODE_FAST) {
                 fa = zmc_fexp_value(zmc_lo(e));
                 fb = zmc_fexp_value(zmc_hi(e));
-            } else {
+            } else if (ZMC_PACKED_EXP_POLY(D_)) {
                 zmc_zexp2(e, fa, fb);
+            } else {      /* packed map and quadratic form, scalar polynomial: fewer live registers at high D */
+                fa = zmc_zexp_value(zmc_lo(e));
+                fb = zmc_zexp_value(zmc_hi(e));
             }
         }
     }
@@ -532,9 +545,15 @@ template <int D> struct ZmcGroup {
 template <class F>
 struct ZmcTune {
     static constexpr int D = F::D;
-    static constexpr bool PACKED = F::HAS_PACKED && ((D == 4) || (D == 6) || (D % 2 == 0 && D <= 8));
+#ifdef ZMC_TUNE_PACKED      /* tuning sweeps override all three from the command line */
+    static constexpr bool PACKED = F::HAS_PACKED && (ZMC_TUNE_PACKED != 0);
+    static constexpr int UNROLL = ZMC_TUNE_UNROLL;
+    static constexpr int MINB = ZMC_TUNE_MINB;
+#else
+    static constexpr bool PACKED = F::HAS_PACKED;
     static constexpr int UNROLL = (D == 4 || D == 6 || D == 12) ? 4 : 2;
     static constexpr int MINB = (D == 4) ? 4 : 3;
+#endif
 };
 
 template <class F>
