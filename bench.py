@@ -204,6 +204,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2_sin6d_depth3_B16")
     ap.add_argument("--math", default="exact", choices=["exact", "fast"])
+    ap.add_argument("--graph", action="store_true", help="replay each step as one CUDA graph (ZMC_OPT_USE_GRAPH)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true")
     args = ap.parse_args()
@@ -232,7 +233,7 @@ def main():
     math = B.MATH_EXACT if args.math == "exact" else B.MATH_FAST
     w_rank = w.with_(seed=w.seed + rank)            # replicas differ only in the seed
     cap = capacity_for(w)
-    it = B.from_workload(w_rank, math=math, max_cells_per_level=cap)
+    it = B.from_workload(w_rank, math=math, max_cells_per_level=cap, use_graph=args.graph)
     it.use_torch_workspace()
     props = torch.cuda.get_device_properties(local_rank)
     n_sm = props.multi_processor_count
@@ -273,6 +274,8 @@ def main():
     samp_ms = sum(st.level[l].sample_ms for l in range(st.levels) if st.level[l].n_cells)
     ctl_ms = sum(st.level[l].control_ms for l in range(st.levels) if st.level[l].n_cells)
     n_sample_launches = sum(1 for l in range(st.levels) if st.level[l].n_cells)
+    if args.graph or samp_ms <= 0:      # a graph replay has no events inside: charge the whole step to the sampling kernel
+        samp_ms = st.total_ms
     achieved = evals_step / (samp_ms * 1e-3)
     peaks = {}
     try:
@@ -295,7 +298,7 @@ def main():
             "dtype": "f32" if w.precision == "f32" else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "note": w.note, "dim": w.dim, "divisions_per_axis": w.g, "samples_per_cell": w.n_samples,
                        "trials": w.trials, "depth": w.depth, "sigma_multiplier": w.sigma_multiplier, "seed": w.seed,
-                       "n_instances": w.n_instances, "max_groups_per_level": w.max_groups_per_level, "math": args.math,
+                       "n_instances": w.n_instances, "max_groups_per_level": w.max_groups_per_level, "math": args.math, "graph": bool(args.graph),
                        "evals_per_step": evals_step, "l2": "256 MiB buffer written between steps (flush); the path reads ~16 B per cell",
                        "parallelism": "replicas x%d" % world},
             "result": {"value": float(value_v[0]), "std": float(value_s[0])},
@@ -338,6 +341,21 @@ def main():
                                                        "evals": int(st3.total_evals),
                                                        "evals_per_s": st3.total_evals / (st3.total_ms * 1e-3)}}
             it3.close()
+            # BASELINE.json configs[0] is launch-bound (microseconds of arithmetic): kernel by kernel vs one CUDA graph
+            w1 = wl["cfg1_sin3d_f64"]
+            for key, graph in (("cfg1_sin3d_f64", False), ("cfg1_sin3d_f64_graph", True)):
+                it1 = B.from_workload(w1, math=math, max_cells_per_level=capacity_for(w1), use_graph=graph)
+                for _ in range(3):
+                    it1.run(stream.cuda_stream)
+                it1.result()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(stream)
+                for _ in range(20):
+                    it1.run(stream.cuda_stream)
+                g1.record(stream)
+                v1, s1 = it1.result()
+                line["time_to_result"][key] = {"ms": g0.elapsed_time(g1) / 20, "value": float(v1[0]), "std": float(s1[0])}
+                it1.close()
 
         if world == 1 and not args.no_cpu_baseline:
             units = max(1, int(2.0e8 // w.n_samples))

@@ -63,8 +63,11 @@ enum {
     ZMC_OPT_KEEP_LEVEL_STATS = 4,     /* 1: keep every level's per-cell arrays for zmc_level_cells (default 0) */
     ZMC_OPT_MAX_CELLS_PER_LEVEL = 5,  /* capacity of one level in cells; 0 = auto (default) */
     ZMC_OPT_GRID_BLOCKS = 6,          /* persistent sampling grid in CTAs; 0 = auto (SM count x resident CTAs) */
-    ZMC_OPT_TARGET_ITEMS = 7          /* a level with fewer (cell,trial) units than this is split into sample chunks
+    ZMC_OPT_TARGET_ITEMS = 7,         /* a level with fewer (cell,trial) units than this is split into sample chunks
                                          until it has about this many work items (default 65536) */
+    ZMC_OPT_USE_GRAPH = 8             /* 1: zmc_run captures its kernel sequence into a CUDA graph once and replays it
+                                         (one launch per run instead of 2 + 6*depth; for launch-bound problems such as
+                                         BASELINE.json configs[0]); per-level times in zmc_stats are then 0 (default 0) */
 };
 enum { ZMC_F64 = 0, ZMC_F32 = 1 };
 enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };

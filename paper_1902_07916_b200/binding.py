@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libzmc.so")
 OK, ERR_ARG, ERR_RANGE, ERR_NO_INTEGRAND, ERR_COMPILE, ERR_CUDA, ERR_CAPACITY, ERR_NOT_RUN, ERR_STATE = 0, -1, -2, -3, -4, -5, -6, -7, -8
 CONST, LINEAR, SIN_SUM, EXP_QUAD, USER = 0, 1, 2, 3, 100
 OPT_PRECISION, OPT_MATH, OPT_MAX_GROUPS_PER_LEVEL, OPT_KEEP_LEVEL_STATS = 1, 2, 3, 4
-OPT_MAX_CELLS_PER_LEVEL, OPT_GRID_BLOCKS, OPT_TARGET_ITEMS = 5, 6, 7
+OPT_MAX_CELLS_PER_LEVEL, OPT_GRID_BLOCKS, OPT_TARGET_ITEMS, OPT_USE_GRAPH = 5, 6, 7, 8
 F64, F32 = 0, 1
 MATH_EXACT, MATH_FAST = 0, 1
 MAX_DEPTH = 15
@@ -241,7 +241,7 @@ class Integrator:
 
 
 def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool = False,
-                  max_cells_per_level: int = 0) -> Integrator:
+                  max_cells_per_level: int = 0, use_graph: bool = False) -> Integrator:
     """zmc_create + zmc_set_integrand + options for one of the seeded workloads."""
     it = Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
     it.set_integrand(_INTEGRAND_ID[w.integrand], w.params, w.n_instances)
@@ -251,6 +251,8 @@ def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool 
         it.set_option(OPT_MAX_GROUPS_PER_LEVEL, w.max_groups_per_level)
     if keep_level_stats:
         it.set_option(OPT_KEEP_LEVEL_STATS, 1)
+    if use_graph:
+        it.set_option(OPT_USE_GRAPH, 1)
     if max_cells_per_level or w.max_cells_per_level:
         it.set_option(OPT_MAX_CELLS_PER_LEVEL, max_cells_per_level or w.max_cells_per_level)
     return it

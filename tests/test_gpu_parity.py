@@ -288,3 +288,56 @@ def test_dimension_above_aot_range_is_jitted():
     it, ores = _run_both(w)
     H.compare_tree(it, ores, w)
     it.close()
+
+
+def test_jit_cache_skips_nvrtc_for_the_same_source():
+    """A second context with the same user source reuses the compiled cubin (process-wide cache keyed by the program text)."""
+    import time
+    w = W.config1()
+    src = USER_SRC.replace("my_f", "my_cached_f")
+    times = []
+    for _ in range(2):
+        it = B.Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
+        t0 = time.perf_counter()
+        it.set_integrand_source(src, "my_cached_f", np.array([[2.0]]), 1)
+        times.append(time.perf_counter() - t0)
+        it.run()
+        v, s = it.result()
+        assert abs(v[0] - 2.0 * H.closed_sin_sum(w.lower, w.upper)) <= 4 * s[0]
+        it.close()
+    assert times[1] < 0.25 * times[0], times
+
+
+def test_graph_mode_is_bit_identical():
+    """ZMC_OPT_USE_GRAPH: the whole run replayed as one CUDA graph gives the same bits as the kernel-by-kernel run,
+    on the default stream and on a side stream, run after run; an option change re-captures."""
+    import torch
+    for w in (W.config1(), W.config2().with_(n_samples=333, depth=3, max_groups_per_level=2)):
+        ref = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 15)
+        ref.run()
+        rv, rs = ref.result()
+        it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 15, use_graph=True)
+        for rep in range(3):
+            it.run()
+            v, s = it.result()
+            assert v[0] == rv[0] and s[0] == rs[0]
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            it.run()
+            v, s = it.result()
+        assert v[0] == rv[0] and s[0] == rs[0]
+        for lev in range(1, w.depth + 1):
+            a, b = it.level_cells(lev), ref.level_cells(lev)
+            np.testing.assert_array_equal(a.S, b.S)
+            np.testing.assert_array_equal(a.refined, b.refined)
+        st = it.stats()
+        assert st.total_ms > 0 and st.level[0].sample_ms == 0.0
+        it.set_option(B.OPT_MAX_GROUPS_PER_LEVEL, 1)          # drops the graph; the next run captures the new parameters
+        it.run()
+        v2, _ = it.result()
+        w1 = w.with_(max_groups_per_level=1)
+        chk = B.from_workload(w1, max_cells_per_level=1 << 15)
+        chk.run()
+        assert v2[0] == chk.result()[0][0]
+        for x in (ref, it, chk):
+            x.close()
