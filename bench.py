@@ -48,6 +48,9 @@ def workloads():
         "cfg1_sin3d_f64": W.config1(),
         # the paper's 12-D Gaussian (Table 4: 47.6 s on one V100), paper's own sizes
         "cfg12_gauss12d": W.gauss12d(),
+        # the paper's own parameter sets (context: 38.7 s and 4.8 s on one V100)
+        "paper_t3_sin6d": W.paper_table3_sin6d(),
+        "paper_t4_gauss9d": W.paper_table4_gauss9d(),
     }
 
 

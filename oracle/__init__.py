@@ -17,6 +17,8 @@ CONST, LINEAR, SIN_SUM, EXP_QUAD = 0, 1, 2, 3
 F64, F32 = 0, 1
 SCOPE_GROUP, SCOPE_POOLED = 0, 1
 BFS, DFS = 0, 1
+SPREAD_TRIALS, SPREAD_SAMPLES = 0, 1              # R13
+BUDGET_PATH_ORDER, BUDGET_LARGEST_SPREAD = 0, 1   # R14
 
 
 class _Cfg(C.Structure):
@@ -25,7 +27,7 @@ class _Cfg(C.Structure):
         ("n_samples", C.c_uint64), ("seed", C.c_uint64), ("sigma_multiplier", C.c_double),
         ("integrand", C.c_int32), ("precision", C.c_int32), ("n_instances", C.c_int32),
         ("params_per_instance", C.c_int32), ("threshold_scope", C.c_int32), ("traversal", C.c_int32),
-        ("max_groups_per_level", C.c_int64),
+        ("max_groups_per_level", C.c_int64), ("spread", C.c_int32), ("budget_order", C.c_int32),
         ("lower", C.POINTER(C.c_double)), ("upper", C.POINTER(C.c_double)), ("params", C.POINTER(C.c_double)),
     ]
 
@@ -54,6 +56,10 @@ def lib():
     L.orc_zexp_value.argtypes = [C.c_float]
     L.orc_zexp_value.restype = C.c_double
     L.orc_unit_sum.argtypes = [C.POINTER(_Cfg), C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, dp, dp]
+    L.orc_unit_sums.argtypes = [C.POINTER(_Cfg), C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, dp, dp]
+    L.orc_cell_stats_samples.argtypes = [dp, dp, C.c_int, C.c_double, C.c_double, C.c_uint64, dp, dp]
+    L.orc_level_sumsq.argtypes = [C.c_void_p, C.c_int, dp]
+    L.orc_level_sumsq.restype = C.c_int64
     L.orc_unit_points.argtypes = [C.POINTER(_Cfg), C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, C.c_uint64, dp, dp]
     L.orc_cell_stats.argtypes = [dp, C.c_int, C.c_double, C.c_double, C.c_uint64, dp, dp, dp]
     L.orc_threshold.argtypes = [dp, C.c_int64, C.c_double]
@@ -101,6 +107,8 @@ class Config:
     threshold_scope: int = SCOPE_GROUP
     traversal: int = BFS
     max_groups_per_level: int = 0
+    spread: int = SPREAD_TRIALS
+    budget_order: int = BUDGET_PATH_ORDER
     _keep: list = field(default_factory=list, repr=False)
 
     def c(self) -> _Cfg:
@@ -115,7 +123,7 @@ class Config:
         self._keep[:] = [lo, up, p]
         return _Cfg(self.dim, self.g, self.trials, self.depth, self.n_samples, self.seed, self.sigma_multiplier,
                     self.integrand, self.precision, self.n_instances, ppi, self.threshold_scope, self.traversal,
-                    self.max_groups_per_level, _dp(lo), _dp(up), _dp(p))
+                    self.max_groups_per_level, self.spread, self.budget_order, _dp(lo), _dp(up), _dp(p))
 
 
 def philox4x32_10(ctr, key):
@@ -196,6 +204,26 @@ def unit_sum(cfg: Config, instance, path, level, coords, trial):
     return S.value, Sabs.value
 
 
+def unit_sums(cfg: Config, instance, path, level, coords, trial):
+    """R13: (S, Q) = (sum f, sum f^2) of one unit."""
+    cc = np.ascontiguousarray(coords, dtype=np.uint32)
+    S, Q = C.c_double(), C.c_double()
+    c = cfg.c()
+    rc = lib().orc_unit_sums(C.byref(c), instance, path & (2**64 - 1), path >> 64, level, _u32p(cc), trial,
+                             C.byref(S), C.byref(Q))
+    if rc != 0:
+        raise ValueError("oracle: bad config")
+    return S.value, Q.value
+
+
+def cell_stats_samples(S, Q, volume, prefactor, n_samples):
+    S = np.ascontiguousarray(S, dtype=np.float64)
+    Q = np.ascontiguousarray(Q, dtype=np.float64)
+    mu, s = C.c_double(), C.c_double()
+    lib().orc_cell_stats_samples(_dp(S), _dp(Q), len(S), volume, prefactor, n_samples, C.byref(mu), C.byref(s))
+    return mu.value, s.value
+
+
 def unit_points(cfg: Config, instance, path, level, coords, trial, n):
     cc = np.ascontiguousarray(coords, dtype=np.uint32)
     x = np.zeros((n, cfg.dim))
@@ -232,6 +260,7 @@ class Level:
     tau: Optional[np.ndarray] = None
     refined: Optional[np.ndarray] = None
     S: Optional[np.ndarray] = None
+    Q: Optional[np.ndarray] = None
 
 
 @dataclass
@@ -270,6 +299,10 @@ def run(cfg: Config, keep_cells: bool = False) -> Result:
                                   _dp(mu), _dp(s), _dp(tau), ref.ctypes.data_as(C.POINTER(C.c_uint8)), _dp(S))
                 rec.instance, rec.mu, rec.s, rec.tau, rec.refined, rec.S = inst, mu, s, tau, ref, S
                 rec.path = [int(phi[i]) << 64 | int(plo[i]) for i in range(n)]
+                if cfg.spread == SPREAD_SAMPLES:
+                    Q = np.zeros((n, cfg.trials))
+                    L.orc_level_sumsq(h, lev, _dp(Q))
+                    rec.Q = Q
             levels.append(rec)
         return Result(value, std, levels, L.orc_total_evals(h))
     finally:

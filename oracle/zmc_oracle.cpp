@@ -16,6 +16,7 @@
  */
 #include "zmc_oracle.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <limits>
@@ -306,6 +307,29 @@ int orc_unit_sum(const orc_config* cfg, uint32_t instance, uint64_t path_lo, uin
     return 0;
 }
 
+/* R13: S and Q = sum_s f*f of one unit (the product is rounded to FP64, then added; sequential order) */
+int orc_unit_sums(const orc_config* cfg, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
+                  const uint32_t* coords, int trial, double* S, double* Q) {
+    if (check_config(cfg)) return -1;
+    const int D = cfg->dim;
+    double lo[64], width[64], V;
+    orc_cell_geometry(D, cfg->lower, cfg->upper, cfg->g, level, coords, lo, width, &V);
+    Integrand F{cfg->integrand, D, cfg->precision, cfg->params + (size_t)instance * cfg->params_per_instance};
+    UnitStream st(cfg->seed, instance, path_lo, path_hi, level, trial);
+    double sum = 0.0, sumsq = 0.0;
+    uint32_t words[64];
+    for (uint64_t s = 0; s < cfg->n_samples; ++s) {
+        for (int d = 0; d < D; ++d) words[d] = st.word(s * (uint64_t)D + (uint64_t)d);
+        double f = eval_point(F, words, lo, width, nullptr);
+        sum = sum + f;
+        double ff = f * f;
+        sumsq = sumsq + ff;
+    }
+    *S = sum;
+    *Q = sumsq;
+    return 0;
+}
+
 int orc_unit_points(const orc_config* cfg, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
                     const uint32_t* coords, int trial, uint64_t n, double* x, double* f) {
     if (check_config(cfg)) return -1;
@@ -347,6 +371,29 @@ void orc_cell_stats(const double* S, int trials, double volume, double prefactor
     if (I) for (int t = 0; t < trials; ++t) I[t] = It[t];
 }
 
+/* R13 (ours): the spread of a cell from its T*N samples instead of from T trial values.
+ * mu is R5's. Pooled sums Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples; population variance of f
+ * var_f = (Qc - Sc^2/M)/M, cut to 0 when the difference is below 2^-40 of Qc (rounding noise of a constant
+ * integrand); s = V*A*sqrt(var_f/M) is the standard error of mu, so sqrt(sum s^2) is a 1-sigma error. */
+void orc_cell_stats_samples(const double* S, const double* Q, int trials, double volume, double prefactor,
+                            uint64_t n_samples, double* mu, double* s) {
+    double VA = volume * prefactor;
+    double acc = 0.0, Sc = 0.0, Qc = 0.0;
+    for (int t = 0; t < trials; ++t) {
+        double v = VA * S[t];
+        acc = acc + v / (double)n_samples;
+        Sc = Sc + S[t];
+        Qc = Qc + Q[t];
+    }
+    *mu = acc / (double)trials;
+    double M = (double)trials * (double)n_samples;
+    double sq = Sc * Sc;
+    double d = Qc - sq / M;
+    if (!(d > Qc * 9.094947017729282e-13)) d = 0.0;     /* 2^-40 */
+    double var_f = d / M;
+    *s = VA * std::sqrt(var_f / M);
+}
+
 /* ------------------------------------------------------------------ R6 */
 /* tau = mean(s) + m * pstd(s) over one set of k stds (two-pass, population form).
  * PAPER.md:71 "determined by the mean and standard deviation of the calculated k standard deviations". */
@@ -376,7 +423,7 @@ struct LevelStore {
     std::vector<uint32_t> instance;
     std::vector<uint64_t> path_lo;
     std::vector<uint32_t> path_hi;
-    std::vector<double> mu, s, tau, S;
+    std::vector<double> mu, s, tau, S, Q;
     std::vector<uint8_t> refined;
     int64_t n_cells = 0, n_refined = 0, n_truncated = 0;
 };
@@ -426,21 +473,26 @@ struct Driver {
         return c;
     }
 
-    /* evaluate one cell at `level`: T trials -> (mu, s)  */
-    void eval_cell(const CellRec& c, int level, double* mu, double* s, double* S_out) {
-        std::vector<double> S(T);
+    /* evaluate one cell at `level`: T trials -> (mu, s) ; PAPER.md:71 (R5), or R13 when spread = samples */
+    void eval_cell(const CellRec& c, int level, double* mu, double* s, double* S_out, double* Q_out) {
+        std::vector<double> S(T), Q(T, 0.0);
         for (int t = 0; t < T; ++t) {
-            orc_unit_sum(cfg, c.instance, (uint64_t)c.path, (uint32_t)(c.path >> 64), level, c.coords.data(), t, &S[t], nullptr);
+            if (cfg->spread == ORC_SPREAD_SAMPLES)
+                orc_unit_sums(cfg, c.instance, (uint64_t)c.path, (uint32_t)(c.path >> 64), level, c.coords.data(), t, &S[t], &Q[t]);
+            else
+                orc_unit_sum(cfg, c.instance, (uint64_t)c.path, (uint32_t)(c.path >> 64), level, c.coords.data(), t, &S[t], nullptr);
         }
         R->evals += (uint64_t)T * cfg->n_samples;
         double lo[64], width[64], V;
         orc_cell_geometry(D, cfg->lower, cfg->upper, g, level, c.coords.data(), lo, width, &V);
         double A = (cfg->integrand == ORC_EXP_QUAD) ? cfg->params[(size_t)c.instance * cfg->params_per_instance] : 1.0;
-        orc_cell_stats(S.data(), T, V, A, cfg->n_samples, nullptr, mu, s);
+        if (cfg->spread == ORC_SPREAD_SAMPLES) orc_cell_stats_samples(S.data(), Q.data(), T, V, A, cfg->n_samples, mu, s);
+        else orc_cell_stats(S.data(), T, V, A, cfg->n_samples, nullptr, mu, s);
         if (S_out) for (int t = 0; t < T; ++t) S_out[t] = S[t];
+        if (Q_out) for (int t = 0; t < T; ++t) Q_out[t] = Q[t];
     }
 
-    void store(int level, const CellRec& c, double mu, double s, double tau, bool refined, const double* S) {
+    void store(int level, const CellRec& c, double mu, double s, double tau, bool refined, const double* S, const double* Q) {
         LevelStore& ls = R->levels[level - 1];
         ls.n_cells++;
         if (refined) ls.n_refined++;
@@ -451,6 +503,7 @@ struct Driver {
         ls.mu.push_back(mu); ls.s.push_back(s); ls.tau.push_back(tau);
         ls.refined.push_back(refined ? 1 : 0);
         for (int t = 0; t < T; ++t) ls.S.push_back(S[t]);
+        if (cfg->spread == ORC_SPREAD_SAMPLES) for (int t = 0; t < T; ++t) ls.Q.push_back(Q[t]);
     }
 
     /* flag rule (R7): level < L and s > tau (strict; NaN compares false), then the budget (R12):
@@ -482,12 +535,12 @@ struct Driver {
         for (int level = 1; level <= L && !parents.empty(); ++level) {
             R->levels_done = level;
             const size_t ng = parents.size();
-            std::vector<double> mu(ng * (size_t)k), s(ng * (size_t)k), S(ng * (size_t)k * (size_t)T);
+            std::vector<double> mu(ng * (size_t)k), s(ng * (size_t)k), S(ng * (size_t)k * (size_t)T), Q(ng * (size_t)k * (size_t)T);
             for (size_t G = 0; G < ng; ++G)
                 for (int64_t j = 0; j < k; ++j) {
                     CellRec c = child(parents[G], j);
                     size_t i = G * (size_t)k + (size_t)j;
-                    eval_cell(c, level, &mu[i], &s[i], &S[i * (size_t)T]);
+                    eval_cell(c, level, &mu[i], &s[i], &S[i * (size_t)T], &Q[i * (size_t)T]);
                 }
             /* thresholds */
             std::vector<double> tau(ng);
@@ -503,14 +556,36 @@ struct Driver {
                     G0 = G1;
                 }
             }
+            /* R7: flagged iff level < L and s > tau (strict; NaN compares false) */
+            const size_t n = ng * (size_t)k;
+            std::vector<char> refine(n, 0);
+            for (size_t i = 0; i < n; ++i) refine[i] = (level < L && s[i] > tau[i / (size_t)k]) ? 1 : 0;
+            /* budget: at most B refined cells per instance and level -- the first B flagged ones in ascending path
+             * order (R12), or the B with the largest spread, equal spreads in path order (R14) */
+            if (cfg->max_groups_per_level > 0) {
+                const size_t B = (size_t)cfg->max_groups_per_level;
+                size_t G0 = 0;
+                while (G0 < ng) {
+                    size_t G1 = G0;
+                    while (G1 < ng && parents[G1].instance == parents[G0].instance) ++G1;
+                    std::vector<size_t> fl;
+                    for (size_t i = G0 * (size_t)k; i < G1 * (size_t)k; ++i) if (refine[i]) fl.push_back(i);
+                    if (fl.size() > B) {
+                        if (cfg->budget_order == ORC_BUDGET_LARGEST_SPREAD)
+                            std::stable_sort(fl.begin(), fl.end(), [&](size_t a, size_t b) { return s[a] > s[b]; });
+                        for (size_t r = B; r < fl.size(); ++r) refine[fl[r]] = 0;
+                        R->levels[level - 1].n_truncated += (int64_t)(fl.size() - B);
+                    }
+                    G0 = G1;
+                }
+            }
             std::vector<CellRec> next;
             for (size_t G = 0; G < ng; ++G)
                 for (int64_t j = 0; j < k; ++j) {
                     size_t i = G * (size_t)k + (size_t)j;
                     CellRec c = child(parents[G], j);
-                    bool refine = decide(level, c.instance, s[i], tau[G]);
-                    store(level, c, mu[i], s[i], tau[G], refine, &S[i * (size_t)T]);
-                    if (refine) next.push_back(c);
+                    store(level, c, mu[i], s[i], tau[G], refine[i] != 0, &S[i * (size_t)T], &Q[i * (size_t)T]);
+                    if (refine[i]) next.push_back(c);
                     else accept(c.instance, mu[i], s[i]);
                 }
             parents.swap(next);
@@ -520,16 +595,16 @@ struct Driver {
     /* ---- depth-first recursion (the paper's picture, Fig. 1); group scope only ---- */
     void refine_dfs(const CellRec& parent, int level) {
         if (level > R->levels_done) R->levels_done = level;
-        std::vector<double> mu((size_t)k), s((size_t)k), S((size_t)k * (size_t)T);
+        std::vector<double> mu((size_t)k), s((size_t)k), S((size_t)k * (size_t)T), Q((size_t)k * (size_t)T);
         std::vector<CellRec> cells;
         for (int64_t j = 0; j < k; ++j) {
             cells.push_back(child(parent, j));
-            eval_cell(cells.back(), level, &mu[j], &s[j], &S[(size_t)j * (size_t)T]);
+            eval_cell(cells.back(), level, &mu[j], &s[j], &S[(size_t)j * (size_t)T], &Q[(size_t)j * (size_t)T]);
         }
         double tau = orc_threshold(s.data(), k, cfg->sigma_multiplier);
         for (int64_t j = 0; j < k; ++j) {
             bool refine = decide(level, cells[j].instance, s[j], tau);
-            store(level, cells[j], mu[j], s[j], tau, refine, &S[(size_t)j * (size_t)T]);
+            store(level, cells[j], mu[j], s[j], tau, refine, &S[(size_t)j * (size_t)T], &Q[(size_t)j * (size_t)T]);
             if (refine) refine_dfs(cells[j], level + 1);
             else accept(cells[j].instance, mu[j], s[j]);
         }
@@ -550,6 +625,9 @@ orc_result* orc_run(const orc_config* cfg, int keep_cells) {
     if (e) { R->err = e; return R; }
     if (cfg->traversal == ORC_DFS && cfg->threshold_scope != ORC_SCOPE_GROUP) {
         R->err = "depth-first traversal needs the per-group threshold"; return R;
+    }
+    if (cfg->traversal == ORC_DFS && cfg->budget_order != ORC_BUDGET_PATH_ORDER && cfg->max_groups_per_level > 0) {
+        R->err = "a largest-spread budget needs a whole level: breadth-first only"; return R;
     }
     Driver drv(cfg, R, keep_cells != 0);
     if (cfg->traversal == ORC_DFS) drv.run_dfs(); else drv.run_bfs();
@@ -584,4 +662,9 @@ int64_t orc_level_cells(const orc_result* r, int level, uint32_t* instance, uint
     }
     if (S) for (size_t i = 0; i < ls.S.size(); ++i) S[i] = ls.S[i];
     return (int64_t)n;
+}
+int64_t orc_level_sumsq(const orc_result* r, int level, double* Q) {
+    const LevelStore& ls = r->levels[level - 1];
+    if (Q) for (size_t i = 0; i < ls.Q.size(); ++i) Q[i] = ls.Q[i];
+    return (int64_t)(ls.Q.size() / (size_t)(r->trials > 0 ? r->trials : 1));
 }

@@ -30,6 +30,8 @@ enum { ORC_CONST = 0, ORC_LINEAR = 1, ORC_SIN_SUM = 2, ORC_EXP_QUAD = 3 };
 enum { ORC_F64 = 0, ORC_F32 = 1 };
 enum { ORC_SCOPE_GROUP = 0, ORC_SCOPE_POOLED = 1 };
 enum { ORC_BFS = 0, ORC_DFS = 1 };
+enum { ORC_SPREAD_TRIALS = 0, ORC_SPREAD_SAMPLES = 1 };   /* R13 */
+enum { ORC_BUDGET_PATH_ORDER = 0, ORC_BUDGET_LARGEST_SPREAD = 1 };   /* R14 */
 
 typedef struct orc_config {
     int32_t dim;                 /* D */
@@ -46,6 +48,8 @@ typedef struct orc_config {
     int32_t threshold_scope;     /* ORC_SCOPE_GROUP (default reading R6) or ORC_SCOPE_POOLED */
     int32_t traversal;           /* ORC_BFS or ORC_DFS (R2: both give the same numbers) */
     int64_t max_groups_per_level;/* R12 refinement budget per instance and level; <= 0 = off */
+    int32_t spread;              /* R13: ORC_SPREAD_TRIALS (the paper, default) or ORC_SPREAD_SAMPLES */
+    int32_t budget_order;        /* R14: which flagged cells the budget keeps: first in path order (R12, default) or largest spread */
     const double* lower;         /* [D] */
     const double* upper;         /* [D] */
     const double* params;        /* [n_instances * params_per_instance] */
@@ -74,6 +78,9 @@ double orc_zexp_value(float e);
 /* ---- one (cell, trial) unit: S = sum_s f(x_s) in FP64, Sabs = sum |f| ---- */
 int orc_unit_sum(const orc_config* cfg, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
                  const uint32_t* coords, int trial, double* S, double* Sabs);
+/* R13: the same unit, also Q = sum_s f(x_s)^2 (FP64: product rounded, then added) */
+int orc_unit_sums(const orc_config* cfg, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
+                  const uint32_t* coords, int trial, double* S, double* Q);
 /* first `n` sample points of a unit (FP64 mode: doubles; FP32 mode: floats widened to double) and f values */
 int orc_unit_points(const orc_config* cfg, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
                     const uint32_t* coords, int trial, uint64_t n, double* x /* [n*D] */, double* f /* [n] */);
@@ -81,6 +88,10 @@ int orc_unit_points(const orc_config* cfg, uint32_t instance, uint64_t path_lo, 
 /* ---- R5: trial estimates -> (mu, s) ; R6: threshold of one set of stds ---- */
 void orc_cell_stats(const double* S, int trials, double volume, double prefactor, uint64_t n_samples,
                     double* I /* [trials] or NULL */, double* mu, double* s);
+/* R13: spread from the samples. mu as in R5; with M = T*N, Sc = sum_t S_t, Qc = sum_t Q_t:
+ *   d = Qc - (Sc*Sc)/M ; d = 0 unless d > Qc * 2^-40 ; s = (V*A) * sqrt((d/M) / M)   -- the standard error of mu */
+void orc_cell_stats_samples(const double* S, const double* Q, int trials, double volume, double prefactor,
+                            uint64_t n_samples, double* mu, double* s);
 double orc_threshold(const double* s, int64_t k, double m);
 
 /* ---- whole tree (R7) ---- */
@@ -96,6 +107,9 @@ uint64_t orc_total_evals(const orc_result*);
 /* kept cells of one level in evaluation order (BFS: ascending (instance, path)); any pointer may be NULL */
 int64_t orc_level_cells(const orc_result*, int level, uint32_t* instance, uint64_t* path_lo, uint32_t* path_hi,
                         double* mu, double* s, double* tau, uint8_t* refined, double* S /* [cells*T] */);
+
+/* R13: per-(cell, trial) sums of squares of one level, [cells*T]; 0 cells unless spread = samples and keep_cells */
+int64_t orc_level_sumsq(const orc_result*, int level, double* Q);
 
 #ifdef __cplusplus
 }

@@ -102,3 +102,18 @@ def gauss12d() -> Workload:
     return Workload("cfg12_gauss12d", 12, (-1.0,) * 12, (1.0,) * 12, 3, 10000, 5, 4, 4.0, 12, EXP_QUAD, F32,
                     params=gaussian_params(12, 0.01), max_cells_per_level=4 * 3 ** 12,
                     note="paper Table 4 (PAPER.md:202-216); f2, Eq. (2), D = 12")
+
+
+def paper_table3_sin6d() -> Workload:
+    """The paper's Table 3 run of f1: 12 divisions per axis (2 985 984 cells), 1e4 samples per cell,
+    5 trials, depth 1 -- 1.49e11 evaluations; 38.7 s on one V100, 298.8 s on one K40m."""
+    return Workload("paper_t3_sin6d", 6, (0.0,) * 6, (10.0,) * 6, 12, 10000, 5, 1, 5.0, 33, SIN_SUM, F32,
+                    note="paper Table 3 (PAPER.md:162-184); f1, Eq. (1)")
+
+
+def paper_table4_gauss9d() -> Workload:
+    """The paper's Table 4 run of f2 in 9-D: 3 divisions per axis, 1e4 samples per cell, 5 trials,
+    depth 4, "4 sigma"; 4.8 s on one V100."""
+    return Workload("paper_t4_gauss9d", 9, (-1.0,) * 9, (1.0,) * 9, 3, 10000, 5, 4, 4.0, 34, EXP_QUAD, F32,
+                    params=gaussian_params(9, 0.01), max_cells_per_level=4 * 3 ** 9,
+                    note="paper Table 4 (PAPER.md:202-216); f2, Eq. (2), D = 9")

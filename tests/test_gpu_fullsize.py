@@ -26,7 +26,7 @@ from tests import helpers as H
 
 pytestmark = pytest.mark.gpu
 
-N_SAMPLED_UNITS = {"cfg2_sin6d_depth3_B16": 24, "cfg3_gauss9d": 40, "cfg4_batched4d_B4": 200, "cfg5_sin6d_level1": 12,
+N_SAMPLED_UNITS = {"cfg2_sin6d_depth3_B16": 24, "cfg2_sin6d_depth2": 16, "cfg3_gauss9d": 40, "cfg4_batched4d_B4": 200, "cfg5_sin6d_level1": 12,
                    "cfg12_gauss12d": 24}
 
 

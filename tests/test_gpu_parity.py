@@ -201,6 +201,19 @@ def test_degenerate_cases():
         it.close()
 
 
+def test_counter_field_limits():
+    """R3 limits: trial index up to 254 (T = 255, 8 bits) and level 15 (4 bits) reach the Philox counter intact."""
+    w = W.Workload("t255", 2, (0.0, 0.0), (1.0, 2.0), 2, 7, 255, 2, 1.0, 77, W.SIN_SUM, W.F32)
+    it, ores = _run_both(w)
+    H.compare_tree(it, ores, w)
+    it.close()
+    w = W.Workload("l15", 1, (0.0,), (3.0,), 2, 9, 3, 15, -1.0, 78, W.SIN_SUM, W.F64, max_groups_per_level=1)
+    it, ores = _run_both(w)
+    H.compare_tree(it, ores, w)
+    assert len(ores.levels) == 15 and it.stats().level[14].n_cells == 2
+    it.close()
+
+
 def test_nan_is_accepted_and_counted():
     """R7: NaN s compares false -> accepted; result NaN; counted in zmc_stats.nonfinite."""
     w = W.Workload("nan", 2, (0.0, 0.0), (1.0, 1.0), 2, 16, 3, 2, 1.0, 1, W.CONST, W.F64, params=np.array([[np.nan]]))
