@@ -91,8 +91,8 @@ def traffic_from_profiles(workload, math):
     return sum(vals) / len(vals) if vals else None
 
 
-def launches_per_step(depth):
-    return 1 + 6 * depth + 1     # init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
+def launches_per_step(depth, by_spread=False):
+    return 1 + (9 if by_spread else 6) * depth + 1     # init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
                                  # (zmc_keys_kernel runs once per context, with the parameter upload)
 
 
@@ -207,6 +207,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2_sin6d_depth3_B16")
     ap.add_argument("--math", default="exact", choices=["exact", "fast"])
+    ap.add_argument("--spread", default="trials", choices=["trials", "samples"], help="DESIGN.md R13")
+    ap.add_argument("--budget-order", default="path", choices=["path", "spread"], help="DESIGN.md R14")
     ap.add_argument("--graph", action="store_true", help="replay each step as one CUDA graph (ZMC_OPT_USE_GRAPH)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true")
@@ -236,7 +238,9 @@ def main():
     math = B.MATH_EXACT if args.math == "exact" else B.MATH_FAST
     w_rank = w.with_(seed=w.seed + rank)            # replicas differ only in the seed
     cap = capacity_for(w)
-    it = B.from_workload(w_rank, math=math, max_cells_per_level=cap, use_graph=args.graph)
+    spread = B.SPREAD_SAMPLES if args.spread == "samples" else B.SPREAD_TRIALS
+    order = B.BUDGET_LARGEST_SPREAD if args.budget_order == "spread" else B.BUDGET_PATH_ORDER
+    it = B.from_workload(w_rank, math=math, max_cells_per_level=cap, use_graph=args.graph, spread=spread, budget_order=order)
     it.use_torch_workspace()
     props = torch.cuda.get_device_properties(local_rank)
     n_sm = props.multi_processor_count
@@ -301,12 +305,12 @@ def main():
             "dtype": "f32" if w.precision == "f32" else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "note": w.note, "dim": w.dim, "divisions_per_axis": w.g, "samples_per_cell": w.n_samples,
                        "trials": w.trials, "depth": w.depth, "sigma_multiplier": w.sigma_multiplier, "seed": w.seed,
-                       "n_instances": w.n_instances, "max_groups_per_level": w.max_groups_per_level, "math": args.math, "graph": bool(args.graph),
+                       "n_instances": w.n_instances, "max_groups_per_level": w.max_groups_per_level, "math": args.math, "graph": bool(args.graph), "spread": args.spread, "budget_order": args.budget_order,
                        "evals_per_step": evals_step, "l2": "256 MiB buffer written between steps (flush); the path reads ~16 B per cell",
                        "parallelism": "replicas x%d" % world},
             "result": {"value": float(value_v[0]), "std": float(value_s[0])},
             "wall_ms_per_step": 1e3 * t_wall / args.steps,
-            "gpu_launches": launches_per_step(w.depth) * args.steps,
+            "gpu_launches": launches_per_step(w.depth, order == B.BUDGET_LARGEST_SPREAD and w.max_groups_per_level > 0) * args.steps,
             "roofline": roofline}
     if clocks is not None:
         line["clocks"] = clocks
@@ -318,7 +322,7 @@ def main():
         t0 = time.perf_counter()
         ev = 0
         for i in range(e2e_steps):
-            it2 = B.from_workload(w_rank, math=math, max_cells_per_level=cap)   # host bounds + params -> zmc_create / zmc_set_integrand
+            it2 = B.from_workload(w_rank, math=math, max_cells_per_level=cap, spread=spread, budget_order=order)   # host bounds + params -> zmc_create / zmc_set_integrand
             it2.use_torch_workspace()
             it2.run(stream.cuda_stream)                                         # parameters H2D + every kernel
             it2.result()                                                         # D2H of (value, std) per instance + overflow flag

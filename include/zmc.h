@@ -65,12 +65,19 @@ enum {
     ZMC_OPT_GRID_BLOCKS = 6,          /* persistent sampling grid in CTAs; 0 = auto (SM count x resident CTAs) */
     ZMC_OPT_TARGET_ITEMS = 7,         /* a level with fewer (cell,trial) units than this is split into sample chunks
                                          until it has about this many work items (default 65536) */
+    ZMC_OPT_SPREAD = 9,               /* ZMC_SPREAD_TRIALS (default, the paper: s = std of the T trial estimates) or
+                                         ZMC_SPREAD_SAMPLES (R13: s = standard error of the cell mean from sum f and
+                                         sum f^2 of its T*N samples; zmc_result's std is then a 1-sigma error) */
+    ZMC_OPT_BUDGET_ORDER = 10,        /* which flagged cells the budget keeps: ZMC_BUDGET_PATH_ORDER (default, R12) or
+                                         ZMC_BUDGET_LARGEST_SPREAD (R14: the B largest s, equal ones in path order) */
     ZMC_OPT_USE_GRAPH = 8             /* 1: zmc_run captures its kernel sequence into a CUDA graph once and replays it
                                          (one launch per run instead of 2 + 6*depth; for launch-bound problems such as
                                          BASELINE.json configs[0]); per-level times in zmc_stats are then 0 (default 0) */
 };
 enum { ZMC_F64 = 0, ZMC_F32 = 1 };
 enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };
+enum { ZMC_SPREAD_TRIALS = 0, ZMC_SPREAD_SAMPLES = 1 };
+enum { ZMC_BUDGET_PATH_ORDER = 0, ZMC_BUDGET_LARGEST_SPREAD = 1 };
 
 typedef struct zmc_ctx zmc_ctx; /* opaque; owned by the library between zmc_create and zmc_destroy */
 
@@ -153,6 +160,10 @@ int zmc_stats(zmc_ctx* ctx, zmc_stats_t* out);
 int zmc_level_cells(zmc_ctx* ctx, int level, uint64_t capacity, uint64_t* n_cells, uint32_t* instance,
                     uint64_t* path_lo, uint32_t* path_hi, double* mu, double* s, double* tau, uint8_t* refined,
                     double* S);
+
+/* Per-(cell, trial) sums of f^2 of one level, Q[c*T + t], FP64 (R13); needs ZMC_OPT_KEEP_LEVEL_STATS and
+ * ZMC_SPREAD_SAMPLES. Q [host] capacity*T doubles, capacity >= the level's cell count. */
+int zmc_level_sumsq(zmc_ctx* ctx, int level, uint64_t capacity, double* Q);
 
 /* Raw generator access for parity tests (R1, R3): n_words words of the flat stream of unit
  * (instance, path, level, trial) starting at word index first_word, produced by the device code.

@@ -23,12 +23,15 @@ OK, ERR_ARG, ERR_RANGE, ERR_NO_INTEGRAND, ERR_COMPILE, ERR_CUDA, ERR_CAPACITY, E
 CONST, LINEAR, SIN_SUM, EXP_QUAD, USER = 0, 1, 2, 3, 100
 OPT_PRECISION, OPT_MATH, OPT_MAX_GROUPS_PER_LEVEL, OPT_KEEP_LEVEL_STATS = 1, 2, 3, 4
 OPT_MAX_CELLS_PER_LEVEL, OPT_GRID_BLOCKS, OPT_TARGET_ITEMS, OPT_USE_GRAPH = 5, 6, 7, 8
+OPT_SPREAD, OPT_BUDGET_ORDER = 9, 10
+SPREAD_TRIALS, SPREAD_SAMPLES = 0, 1
+BUDGET_PATH_ORDER, BUDGET_LARGEST_SPREAD = 0, 1
 F64, F32 = 0, 1
 MATH_EXACT, MATH_FAST = 0, 1
 MAX_DEPTH = 15
 
 EXPORTS = ["zmc_create", "zmc_set_integrand", "zmc_set_integrand_source", "zmc_set_option", "zmc_workspace_bytes",
-           "zmc_set_workspace", "zmc_run", "zmc_result", "zmc_stats", "zmc_level_cells", "zmc_debug_words",
+           "zmc_set_workspace", "zmc_run", "zmc_result", "zmc_stats", "zmc_level_cells", "zmc_level_sumsq", "zmc_debug_words",
            "zmc_debug_points", "zmc_microbench", "zmc_last_error", "zmc_status_string", "zmc_destroy"]
 
 _INTEGRAND_ID = {W.CONST: CONST, W.LINEAR: LINEAR, W.SIN_SUM: SIN_SUM, W.EXP_QUAD: EXP_QUAD}
@@ -79,6 +82,7 @@ def lib():
     L.zmc_result.argtypes = [vp, dp, dp]
     L.zmc_stats.argtypes = [vp, C.POINTER(Stats)]
     L.zmc_level_cells.argtypes = [vp, C.c_int, C.c_uint64, u64p, u32p, u64p, u32p, dp, dp, dp, C.POINTER(C.c_uint8), dp]
+    L.zmc_level_sumsq.argtypes = [vp, C.c_int, C.c_uint64, dp]
     L.zmc_debug_words.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_uint64, C.c_uint64, u32p]
     L.zmc_debug_points.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, C.c_uint64, dp, dp]
     L.zmc_microbench.argtypes = [C.c_int, vp, dp, dp]
@@ -225,6 +229,11 @@ class Integrator:
         path = [(int(h) << 64) | int(l) for h, l in zip(phi, plo)]
         return LevelCells(inst, path, mu, s, tau, ref, S)
 
+    def level_sumsq(self, level: int, n_cells: int) -> np.ndarray:
+        Q = np.zeros((n_cells, self.trials))
+        self._check(self._L.zmc_level_sumsq(self._h, level, n_cells, _dp(Q)))
+        return Q
+
     def debug_words(self, instance: int, path: int, level: int, trial: int, first_word: int, n_words: int) -> np.ndarray:
         out = np.zeros(n_words, dtype=np.uint32)
         self._check(self._L.zmc_debug_words(self._h, instance, path & (2 ** 64 - 1), path >> 64, level, trial,
@@ -241,7 +250,8 @@ class Integrator:
 
 
 def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool = False,
-                  max_cells_per_level: int = 0, use_graph: bool = False) -> Integrator:
+                  max_cells_per_level: int = 0, use_graph: bool = False, spread: int = SPREAD_TRIALS,
+                  budget_order: int = BUDGET_PATH_ORDER) -> Integrator:
     """zmc_create + zmc_set_integrand + options for one of the seeded workloads."""
     it = Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
     it.set_integrand(_INTEGRAND_ID[w.integrand], w.params, w.n_instances)
@@ -253,6 +263,10 @@ def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool 
         it.set_option(OPT_KEEP_LEVEL_STATS, 1)
     if use_graph:
         it.set_option(OPT_USE_GRAPH, 1)
+    if spread != SPREAD_TRIALS:
+        it.set_option(OPT_SPREAD, spread)
+    if budget_order != BUDGET_PATH_ORDER:
+        it.set_option(OPT_BUDGET_ORDER, budget_order)
     if max_cells_per_level or w.max_cells_per_level:
         it.set_option(OPT_MAX_CELLS_PER_LEVEL, max_cells_per_level or w.max_cells_per_level)
     return it

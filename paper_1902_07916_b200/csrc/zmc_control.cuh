@@ -61,6 +61,18 @@ struct ZmcCtlArgs {
     double* var;            /* [instance] */
     zu64* nonfinite;
     zu32* overflow;
+    /* R13: spread from the samples */
+    zu32 spread;            /* 0: from the T trial values (paper) ; 1: from sum f, sum f^2 of the T*N samples */
+    const double* partial_q;
+    double* Q;              /* [cell*T + t], or nullptr */
+    /* R14: the budget keeps the largest spreads */
+    zu32 budget_order;      /* 0: first B flagged cells in path order (R12) ; 1: the B largest spreads */
+    zu64* piv;              /* [instance] key (bits of s) of the B-th largest flagged spread; 0 = keep every flagged cell */
+    zu64* quota;            /* [instance] how many cells with s == pivot are kept (the first in path order) */
+    zu64* cnt_gt;           /* [group] flagged cells with key > pivot */
+    zu64* cnt_eq;           /* [group] flagged cells with key == pivot */
+    zu64* excl_gt;          /* [group] exclusive prefixes over all groups */
+    zu64* excl_eq;
 };
 
 /* plan of one level: how the (cell, trial) units are cut into work items */
@@ -146,14 +158,33 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const _
             acc = __dadd_rn(acc, __ddiv_rn(__dmul_rn(VA, S), dN));
         }
         const double mu = __ddiv_rn(acc, dT);
-        double q = 0.0;
-        for (zu32 t = 0; t < c.T; ++t) {
-            double S = p[(zu64)t * nch];
-            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)t * nch + ch]);
-            const double d = __dadd_rn(__ddiv_rn(__dmul_rn(VA, S), dN), -mu);
-            q = __dadd_rn(q, __dmul_rn(d, d));
+        double sd;
+        if (c.spread == 0) {
+            double q = 0.0;
+            for (zu32 t = 0; t < c.T; ++t) {
+                double S = p[(zu64)t * nch];
+                for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)t * nch + ch]);
+                const double d = __dadd_rn(__ddiv_rn(__dmul_rn(VA, S), dN), -mu);
+                q = __dadd_rn(q, __dmul_rn(d, d));
+            }
+            sd = __dsqrt_rn(__ddiv_rn(q, dT));
+        } else {
+            /* R13: Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples ; d = Qc - Sc^2/M, 0 unless d > Qc*2^-40 ;
+             * s = (V*A) * sqrt((d/M)/M), the standard error of mu */
+            const double* pq = c.partial_q + cell * (zu64)c.T * nch;
+            double Sc = 0.0, Qc = 0.0;
+            for (zu32 t = 0; t < c.T; ++t) {
+                double S = p[(zu64)t * nch], Q = pq[(zu64)t * nch];
+                for (zu32 ch = 1; ch < nch; ++ch) { S = __dadd_rn(S, p[(zu64)t * nch + ch]); Q = __dadd_rn(Q, pq[(zu64)t * nch + ch]); }
+                if (c.Q) c.Q[cell * c.T + t] = Q;
+                Sc = __dadd_rn(Sc, S);
+                Qc = __dadd_rn(Qc, Q);
+            }
+            const double M = __dmul_rn(dT, dN);
+            double d = __dadd_rn(Qc, -__ddiv_rn(__dmul_rn(Sc, Sc), M));
+            if (!(d > __dmul_rn(Qc, 9.094947017729282e-13))) d = 0.0;
+            sd = __dmul_rn(VA, __dsqrt_rn(__ddiv_rn(__ddiv_rn(d, M), M)));
         }
-        const double sd = __dsqrt_rn(__ddiv_rn(q, dT));
         c.mu[cell] = mu;
         c.s[cell] = sd;
         if (!(fabs(mu) <= 1.7976931348623157e308) || !(fabs(sd) <= 1.7976931348623157e308)) ++bad;
@@ -298,25 +329,123 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid
     }
 }
 
+/* ------------------------------------------------------------------ R14: the budget keeps the largest spreads */
+/* One block per instance: if more than B cells are flagged, radix-select (8 passes of 8 bits over the bit pattern
+ * of s, which orders positive doubles) the B-th largest flagged spread -> piv, and how many cells equal to it are
+ * kept -> quota = B - #(s > pivot). Otherwise piv = 0: every flagged cell has s > tau >= 0, i.e. key > 0. */
+__global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ zu32 hist[256];
+    __shared__ zu64 sh_prefix, sh_need, sh_above;
+    for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
+        const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
+        const zu64 cb = (g1 > g0) ? c.excl[g1 - 1] + c.cnt[g1 - 1] - c.excl[g0] : 0ull;
+        __syncthreads();
+        if (cb <= c.budget) {
+            if (threadIdx.x == 0) { c.piv[b] = 0ull; c.quota[b] = 0ull; }
+            continue;
+        }
+        if (threadIdx.x == 0) { sh_prefix = 0ull; sh_need = c.budget; sh_above = 0ull; }
+        for (int pass = 7; pass >= 0; --pass) {
+            const int shift = pass * 8;
+            for (int i = threadIdx.x; i < 256; i += ZMC_SCAN_THREADS) hist[i] = 0u;
+            __syncthreads();
+            const zu64 prefix = sh_prefix;
+            for (zu64 cell = g0 * c.k + threadIdx.x; cell < g1 * c.k; cell += ZMC_SCAN_THREADS) {
+                const double sj = c.s[cell];
+                if (sj > c.tau[cell / c.k]) {
+                    const zu64 key = (zu64)__double_as_longlong(sj);
+                    if (pass == 7 || (key >> (shift + 8)) == (prefix >> (shift + 8))) atomicAdd(&hist[(key >> shift) & 255ull], 1u);
+                }
+            }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                zu64 cum = 0, need = sh_need;
+                int digit = 0;
+                for (int dgt = 255; dgt >= 0; --dgt) {
+                    if (cum + hist[dgt] >= need) { digit = dgt; break; }
+                    cum += hist[dgt];
+                }
+                sh_need = need - cum;        /* rank, from the top, inside the chosen bin */
+                sh_above += cum;             /* keys strictly greater than everything in the chosen bin */
+                sh_prefix = prefix | ((zu64)digit << shift);
+            }
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) { c.piv[b] = sh_prefix; c.quota[b] = c.budget - sh_above; }
+    }
+}
+
+/* per sibling group: flagged cells above and at the instance's pivot */
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_count2_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    const zu64 n_groups = c.info[c.level].n_groups;
+    for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
+        const double* s = c.s + G * c.k;
+        const double tau = c.tau[G];
+        const zu64 piv = c.piv[c.cur.inst[G]];
+        zu64 ngt = 0, neq = 0;
+        if (c.level < c.L)
+            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS)
+                if (s[j] > tau) {
+                    const zu64 key = (zu64)__double_as_longlong(s[j]);
+                    ngt += (key > piv) ? 1ull : 0ull;
+                    neq += (key == piv) ? 1ull : 0ull;
+                }
+        ngt = zmc_block_sum_u64(ngt, smem_u);
+        neq = zmc_block_sum_u64(neq, smem_u);
+        if (threadIdx.x == 0) { c.cnt_gt[G] = ngt; c.cnt_eq[G] = neq; }
+    }
+}
+
+/* One block: exclusive scans of cnt_gt and cnt_eq over the groups. */
+__global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ zu64 warp_tot[32];
+    __shared__ zu64 total;
+    __shared__ zu64 carry;
+    const zu64 n_groups = c.info[c.level].n_groups;
+    for (int which = 0; which < 2; ++which) {
+        const zu64* in = which ? c.cnt_eq : c.cnt_gt;
+        zu64* out = which ? c.excl_eq : c.excl_gt;
+        __syncthreads();
+        if (threadIdx.x == 0) carry = 0;
+        __syncthreads();
+        for (zu64 base = 0; base < n_groups; base += ZMC_SCAN_THREADS) {
+            const zu64 G = base + threadIdx.x;
+            const zu64 v = (G < n_groups) ? in[G] : 0ull;
+            const zu64 ex = zmc_scan_block_excl(v, warp_tot, &total);
+            if (G < n_groups) out[G] = carry + ex;
+            __syncthreads();
+            if (threadIdx.x == 0) carry += total;
+            __syncthreads();
+        }
+    }
+}
+
 /* R7: one block per sibling group. Flagged cells get their rank within the instance (stable, path
  * order); rank < B (R12) and slot < capacity -> the child record (R2) is written to the next parent
  * list. Every other cell is accepted: its mu and s^2 go into the group's fixed-shape sums. */
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
-    __shared__ zu32 warp_cnt[ZMC_CTL_THREADS / 32];
-    __shared__ zu64 run;
+    __shared__ zu32 warp_cnt[ZMC_CTL_THREADS / 32], warp_cnt_eq[ZMC_CTL_THREADS / 32];
+    __shared__ zu64 run, run_eq;
     const zu64 n_groups = c.info[c.level].n_groups;
     const zu32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
         const zu32 inst = c.cur.inst[G];
         const double tau = c.tau[G];
-        const zu64 r0 = c.excl[G] - c.excl[c.gfirst[inst]];   /* flagged cells of this instance in earlier groups */
+        const bool by_spread = (c.budget_order != 0) && (c.budget != ~0ull);
+        const zu64 gf = c.gfirst[inst];
+        const zu64 r0 = c.excl[G] - c.excl[gf];   /* flagged cells of this instance in earlier groups */
+        const zu64 r0_gt = by_spread ? c.excl_gt[G] - c.excl_gt[gf] : 0ull;   /* ... above the pivot */
+        const zu64 r0_eq = by_spread ? c.excl_eq[G] - c.excl_eq[gf] : 0ull;   /* ... at the pivot */
+        const zu64 piv = by_spread ? c.piv[inst] : 0ull;
+        const zu64 quota = by_spread ? c.quota[inst] : 0ull;
         const zu64 slot0 = c.out0[inst];
         const zu64 plo = c.cur.plo[G];
         const zu32 phi = c.cur.phi[G];
         double acc_mu = 0.0, acc_var = 0.0;
         __syncthreads();
-        if (threadIdx.x == 0) run = 0;
+        if (threadIdx.x == 0) { run = 0; run_eq = 0; }
         __syncthreads();
         for (zu64 base = 0; base < c.k; base += ZMC_CTL_THREADS) {
             const zu64 j = base + threadIdx.x;
@@ -328,19 +457,37 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
                 muj = c.mu[cell];
                 flag = (c.level < c.L) && (sj > tau);
             }
-            const zu32 bal = __ballot_sync(0xFFFFFFFFu, flag);
-            if (lane == 0) warp_cnt[warp] = __popc(bal);
+            /* path order: every flagged cell counts in `run`. Largest spread: cells above the pivot count in `run`,
+             * cells at the pivot in `run_eq`; cells below it are not candidates. */
+            const zu64 key = (zu64)__double_as_longlong(sj);
+            const bool is_eq = by_spread && flag && key == piv;
+            const bool is_a = by_spread ? (flag && key > piv) : flag;
+            const zu32 bal = __ballot_sync(0xFFFFFFFFu, is_a);
+            const zu32 bal_eq = __ballot_sync(0xFFFFFFFFu, is_eq);
+            if (lane == 0) { warp_cnt[warp] = __popc(bal); warp_cnt_eq[warp] = __popc(bal_eq); }
             __syncthreads();
-            zu64 before = run;
-            zu32 tile_total = 0;
+            zu64 before = run, before_eq = run_eq;
+            zu32 tile_total = 0, tile_total_eq = 0;
 #pragma unroll
             for (int w = 0; w < ZMC_CTL_THREADS / 32; ++w) {
-                if ((zu32)w < warp) before += warp_cnt[w];
+                if ((zu32)w < warp) { before += warp_cnt[w]; before_eq += warp_cnt_eq[w]; }
                 tile_total += warp_cnt[w];
+                tile_total_eq += warp_cnt_eq[w];
             }
-            const zu64 rank = r0 + before + __popc(bal & ((1u << lane) - 1u));
+            const zu32 below = (1u << lane) - 1u;
+            zu64 rank;          /* position among the cells that are kept, in path order */
+            bool want;
+            if (by_spread) {
+                const zu64 n_gt = r0_gt + before + __popc(bal & below);
+                const zu64 n_eq = r0_eq + before_eq + __popc(bal_eq & below);
+                want = is_a || (is_eq && n_eq < quota);
+                rank = n_gt + (n_eq < quota ? n_eq : quota);
+            } else {
+                rank = r0 + before + __popc(bal & below);
+                want = flag && rank < c.budget;
+            }
             bool kept = false;
-            if (flag && rank < c.budget) {
+            if (want) {
                 const zu64 slot = slot0 + rank;
                 if (slot < c.cap_par) {
                     kept = true;
@@ -364,7 +511,7 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
                 if (c.refined) c.refined[cell] = kept ? 1 : 0;
             }
             __syncthreads();
-            if (threadIdx.x == 0) run += tile_total;
+            if (threadIdx.x == 0) { run += tile_total; run_eq += tile_total_eq; }
             __syncthreads();
         }
         const double gm = zmc_block_sum(acc_mu, smem);

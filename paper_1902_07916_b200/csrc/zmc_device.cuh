@@ -58,6 +58,7 @@ struct ZmcSampleArgs {
     zu64 par_stride;
     ZmcLevelInfo* info;      /* this level's */
     double* partial;         /* [item] FP64 partial sums, item = (cell*T + trial)*n_chunks + chunk */
+    double* partial_q;       /* [item] FP64 partial sums of f^2 (SQ kernels only: R13) */
     const zu32* keys;        /* [instance][2] derived Philox keys (R3) */
     const double* params;    /* [instance][ppi] */
     const float* params_f32; /* the same rounded to FP32 (user integrands) */
@@ -314,6 +315,7 @@ struct ZmcIntegrand;
 template <int ID, int D_, int MODE>
 struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
     static constexpr int D = D_;
+    static constexpr int PREC = ZMC_PREC_F32;
     ZmcMapF32<D_> map;
     float c0;           /* CONST/LINEAR: p[0] ; EXP_QUAD: -a */
     float lin[ID == ZMC_ID_LINEAR ? D_ : 1];
@@ -426,6 +428,7 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
 template <int ID, int D_, int MODE>
 struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
     static constexpr int D = D_;
+    static constexpr int PREC = ZMC_PREC_F64;
     ZmcMapF64<D_> map;
     double c0;          /* CONST/LINEAR: p[0] ; EXP_QUAD: a */
     double aux[(ID == ZMC_ID_LINEAR || ID == ZMC_ID_EXP_QUAD) ? D_ : 1];   /* LINEAR: coefficients ; EXP_QUAD: centre */
@@ -556,9 +559,16 @@ struct ZmcTune {
 #endif
 };
 
+/* R13: q + f*f. FP32-mode values have 24 significant bits, so the product is exact and one DFMA is the
+ * rounded-product-then-add of the definition; FP64 values get the two operations. */
 template <class F>
+__device__ __forceinline__ double zmc_sq_add(double q, double f) {
+    return (F::PREC == ZMC_PREC_F32) ? __fma_rn(f, f, q) : __dadd_rn(q, __dmul_rn(f, f));
+}
+
+template <class F, bool SQ>
 __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
-                                               double* acc) {
+                                               double* acc, double* accq) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     zu32 w[4 * CG];
     const zu32 q0 = gi * (zu32)CG;
@@ -571,17 +581,22 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
             f.eval2(&w[s * D], &w[(s + 1) * D], fa, fb);
             acc[s] = __dadd_rn(acc[s], fa);
             acc[s + 1] = __dadd_rn(acc[s + 1], fb);
+            if (SQ) { accq[s] = zmc_sq_add<F>(accq[s], fa); accq[s + 1] = zmc_sq_add<F>(accq[s + 1], fb); }
         }
     } else {
 #pragma unroll
-        for (int s = 0; s < SG; ++s) acc[s] = __dadd_rn(acc[s], f.eval(&w[s * D], nullptr));
+        for (int s = 0; s < SG; ++s) {
+            const double fv = f.eval(&w[s * D], nullptr);
+            acc[s] = __dadd_rn(acc[s], fv);
+            if (SQ) accq[s] = zmc_sq_add<F>(accq[s], fv);
+        }
     }
 }
 
 /* groups gi and gj: acc[0..SG) takes gi's samples, acc[SG..2SG) gj's -- the same sums as two zmc_group_eval calls */
-template <class F>
+template <class F, bool SQ>
 __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
-                                                    zu32 gj, double* acc) {
+                                                    zu32 gj, double* acc, double* accq) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     if (ZmcTune<F>::PACKED && SG == 1) {      /* one sample per group (D = 4, 8, ..): pack across the two groups */
         zu32 wa[4 * CG], wb[4 * CG];
@@ -593,16 +608,18 @@ __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySche
         f.eval2(wa, wb, fa, fb);
         acc[0] = __dadd_rn(acc[0], fa);
         acc[1] = __dadd_rn(acc[1], fb);
+        if (SQ) { accq[0] = zmc_sq_add<F>(accq[0], fa); accq[1] = zmc_sq_add<F>(accq[1], fb); }
     } else {
-        zmc_group_eval(f, ks, uc, gi, acc);
-        zmc_group_eval(f, ks, uc, gj, acc + SG);
+        zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq);
+        zmc_group_eval<F, SQ>(f, ks, uc, gj, acc + SG, accq + SG);
     }
 }
 
 /* UKEY: every work item has the same Philox key (n_instances == 1); it comes from the kernel
  * parameters (constant bank), so the ten round keys live in uniform registers: 20 fewer registers
  * per thread and one register operand fewer on every Philox LOP3. */
-template <class F, bool UKEY>
+/* SQ (R13): also sum f^2 per unit, into partial_q. */
+template <class F, bool UKEY, bool SQ = false>
 __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     const zu32 lane = threadIdx.x & 31u;
@@ -636,18 +653,18 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
 
         /* lanes stride over the chunk's groups; acc[0..SG) sums the groups at even multiples of 32 from the
          * lane's first one, acc[SG..2SG) those at odd multiples -- whatever UNROLL is, so results do not depend on it */
-        double acc[2 * SG];
+        double acc[2 * SG], accq[2 * SG];
 #pragma unroll
-        for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
+        for (int s = 0; s < 2 * SG; ++s) { acc[s] = 0.0; accq[s] = 0.0; }
         zu32 gi = gb + lane;
         if (ZmcTune<F>::UNROLL == 4) {
             for (; gi + 96u < gfe; gi += 128u) {
-                zmc_group_eval_pair(f, ks, uc, gi, gi + 32u, acc);
-                zmc_group_eval_pair(f, ks, uc, gi + 64u, gi + 96u, acc);
+                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq);
+                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi + 64u, gi + 96u, acc, accq);
             }
         }
-        for (; gi + 32u < gfe; gi += 64u) zmc_group_eval_pair(f, ks, uc, gi, gi + 32u, acc);
-        if (gi < gfe) zmc_group_eval(f, ks, uc, gi, acc);
+        for (; gi + 32u < gfe; gi += 64u) zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq);
+        if (gi < gfe) zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq);
         if (tail != 0u && ge > full_groups && lane == 0u) {   /* the partial group: only its first `tail` samples exist */
             zu32 w[4 * CG];
             const zu32 q0 = full_groups * (zu32)CG;
@@ -655,13 +672,25 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
             for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
 #pragma unroll
             for (int s = 0; s < SG; ++s)
-                if ((zu32)s < tail) acc[s] = __dadd_rn(acc[s], f.eval(&w[s * D], nullptr));
+                if ((zu32)s < tail) {
+                    const double fv = f.eval(&w[s * D], nullptr);
+                    acc[s] = __dadd_rn(acc[s], fv);
+                    if (SQ) accq[s] = zmc_sq_add<F>(accq[s], fv);
+                }
         }
         double sum = acc[0];
 #pragma unroll
         for (int s = 1; s < 2 * SG; ++s) sum = __dadd_rn(sum, acc[s]);
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
+        if (SQ) {
+            double sq = accq[0];
+#pragma unroll
+            for (int s = 1; s < 2 * SG; ++s) sq = __dadd_rn(sq, accq[s]);
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) sq = __dadd_rn(sq, __shfl_down_sync(0xFFFFFFFFu, sq, off));
+            if (lane == 0u) a.partial_q[item] = sq;
+        }
         if (lane == 0u) a.partial[item] = sum;
     }
 }

@@ -106,10 +106,10 @@ def compare_tree(it, ores, w: W.Workload, *, tol_sum=1e-12, tol_stat=1e-11, exac
     return n_cmp
 
 
-def host_control(mu, s, k, level, depth, m, instance, budget=0):
+def host_control(mu, s, k, level, depth, m, instance, budget=0, largest_spread=False):
     """Re-derive the control path (H7-H10) of one level in numpy from dumped per-cell (mu, s):
     per-group tau = mean + m*pstd (R6), flags s > tau for level < depth (R7), first-B budget per
-    instance in path order (R12), accepted sums. Test-side restatement; shares nothing with either
+    instance in path order (R12) or largest-spread-first (R14), accepted sums. Test-side restatement; shares nothing with either
     implementation. Returns (tau_per_cell, refined, acc_value[instance], acc_var[instance])."""
     n = len(mu)
     G = n // k
@@ -123,6 +123,8 @@ def host_control(mu, s, k, level, depth, m, instance, budget=0):
     if budget > 0:
         for b in np.unique(instance):
             idx = np.nonzero(flag & (instance == b))[0]
+            if largest_spread:      # R14: the B largest spreads, equal ones in path order
+                idx = np.array(sorted(idx, key=lambda i: (-s[i], i)), dtype=np.int64)
             refined[idx[budget:]] = False
     ninst = int(instance.max()) + 1
     val = np.zeros(ninst)

@@ -207,7 +207,7 @@ def test_counter_field_limits():
     it, ores = _run_both(w)
     H.compare_tree(it, ores, w)
     it.close()
-    w = W.Workload("l15", 1, (0.0,), (3.0,), 2, 9, 3, 15, -1.0, 78, W.SIN_SUM, W.F64, max_groups_per_level=1)
+    w = W.Workload("l15", 1, (0.0,), (3.0,), 2, 9, 3, 15, 0.0, 78, W.SIN_SUM, W.F64)
     it, ores = _run_both(w)
     H.compare_tree(it, ores, w)
     assert len(ores.levels) == 15 and it.stats().level[14].n_cells == 2
