@@ -555,7 +555,7 @@ struct ZmcTune {
 #else
     static constexpr bool PACKED = F::HAS_PACKED;
     static constexpr int UNROLL = (D == 4 || D == 6 || D == 12) ? 4 : 2;
-    static constexpr int MINB = (D == 4) ? 4 : 3;
+    static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && D >= 7) ? 2 : ((D == 4) ? 4 : 3);   /* FP64 at high D spills below 255 registers */
 #endif
 };
 
