@@ -207,6 +207,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2_sin6d_depth3_B16")
     ap.add_argument("--math", default="exact", choices=["exact", "fast"])
+    ap.add_argument("--precision", default="workload", choices=["workload", "f32", "f64"], help="override the workload's evaluation precision")
     ap.add_argument("--spread", default="trials", choices=["trials", "samples"], help="DESIGN.md R13")
     ap.add_argument("--budget-order", default="path", choices=["path", "spread"], help="DESIGN.md R14")
     ap.add_argument("--graph", action="store_true", help="replay each step as one CUDA graph (ZMC_OPT_USE_GRAPH)")
@@ -217,6 +218,8 @@ def main():
         args.warmup = 3
     wl = workloads()
     w = wl[args.workload]
+    if args.precision != "workload":
+        w = w.with_(precision=args.precision)
 
     if args.impl == "reference":
         run_reference(args, w, args.workload)
