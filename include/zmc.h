@@ -65,14 +65,14 @@ enum {
     ZMC_OPT_GRID_BLOCKS = 6,          /* persistent sampling grid in CTAs; 0 = auto (SM count x resident CTAs) */
     ZMC_OPT_TARGET_ITEMS = 7,         /* a level with fewer (cell,trial) units than this is split into sample chunks
                                          until it has about this many work items (default 65536) */
+    ZMC_OPT_USE_GRAPH = 8,            /* 1: zmc_run captures its kernel sequence into a CUDA graph once and replays it
+                                         (one launch per run instead of 2 + 6*depth; for launch-bound problems such as
+                                         BASELINE.json configs[0]); per-level times in zmc_stats are then 0 (default 0) */
     ZMC_OPT_SPREAD = 9,               /* ZMC_SPREAD_TRIALS (default, the paper: s = std of the T trial estimates) or
                                          ZMC_SPREAD_SAMPLES (R13: s = standard error of the cell mean from sum f and
                                          sum f^2 of its T*N samples; zmc_result's std is then a 1-sigma error) */
-    ZMC_OPT_BUDGET_ORDER = 10,        /* which flagged cells the budget keeps: ZMC_BUDGET_PATH_ORDER (default, R12) or
+    ZMC_OPT_BUDGET_ORDER = 10         /* which flagged cells the budget keeps: ZMC_BUDGET_PATH_ORDER (default, R12) or
                                          ZMC_BUDGET_LARGEST_SPREAD (R14: the B largest s, equal ones in path order) */
-    ZMC_OPT_USE_GRAPH = 8             /* 1: zmc_run captures its kernel sequence into a CUDA graph once and replays it
-                                         (one launch per run instead of 2 + 6*depth; for launch-bound problems such as
-                                         BASELINE.json configs[0]); per-level times in zmc_stats are then 0 (default 0) */
 };
 enum { ZMC_F64 = 0, ZMC_F32 = 1 };
 enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };

@@ -4,9 +4,12 @@
  *
  *   zmc_keys_kernel        derived Philox keys, one call per instance                           (R3)
  *   zmc_init_kernel        root parents, zeroed results, level-1 plan
- *   zmc_cell_stats_kernel  per-(cell,trial) partial sums -> S_t -> I_t -> (mu_c, s_c)          (R5)
+ *   zmc_cell_stats_kernel  per-(cell,trial) partial sums -> S_t -> I_t -> (mu_c, s_c)          (R5; R13 from sum f^2)
  *   zmc_threshold_kernel   per sibling group: tau = mean(s) + m*pstd(s), number of s > tau      (R6)
  *   zmc_scan_kernel        exclusive scans over groups and instances -> output slots, next plan (R7, R12)
+ *   zmc_select_kernel, zmc_count2_kernel, zmc_scan2_kernel
+ *                          only with ZMC_BUDGET_LARGEST_SPREAD: radix select of the B largest flagged
+ *                          spreads per instance, counts above / at the pivot, their scans            (R14)
  *   zmc_scatter_kernel     stable compaction of flagged cells into the next parent list;
  *                          accepted cells -> per-group (sum mu, sum s^2)                         (R7)
  *   zmc_accumulate_kernel  per instance: value += sum mu, var += sum s^2                         (R7)

@@ -7,6 +7,12 @@
  * from a device counter whose bound was written by the previous level's control kernels, so the
  * host enqueues all levels up front.
  *
+ * What bounds it: the 32x32->64-bit multiplies of Philox, IMAD.WIDE.U32, run
+ * only on the FMA-heavy pipe (4 clocks per warp-instruction), and next to them nothing issues for
+ * free. So the kernel is built to issue as few other instructions as possible: two samples per
+ * packed FP32 instruction (FFMA2/FADD2/FMUL2), round keys in uniform registers when the launch has
+ * one key (UKEY), 2 or 4 sample groups per loop trip, per-dimension choices in ZmcTune.
+ *
  * This file is self-contained (no #include) because it is compiled twice: ahead of time by nvcc
  * for the built-in integrands (zmc_inst_*.cu) and at run time by NVRTC for user integrands and
  * for dimensions without a pre-compiled instance (zmc_lib.cu embeds this text).
