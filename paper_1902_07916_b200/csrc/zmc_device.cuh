@@ -587,14 +587,14 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
             f.eval2(&w[s * D], &w[(s + 1) * D], fa, fb);
             acc[s] = __dadd_rn(acc[s], fa);
             acc[s + 1] = __dadd_rn(acc[s + 1], fb);
-            if (SQ) { accq[s] = zmc_sq_add<F>(accq[s], fa); accq[s + 1] = zmc_sq_add<F>(accq[s + 1], fb); }
+            if (SQ) { accq[0] = zmc_sq_add<F>(accq[0], fa); accq[1] = zmc_sq_add<F>(accq[1], fb); }
         }
     } else {
 #pragma unroll
         for (int s = 0; s < SG; ++s) {
             const double fv = f.eval(&w[s * D], nullptr);
             acc[s] = __dadd_rn(acc[s], fv);
-            if (SQ) accq[s] = zmc_sq_add<F>(accq[s], fv);
+            if (SQ) accq[s & 1] = zmc_sq_add<F>(accq[s & 1], fv);
         }
     }
 }
@@ -617,7 +617,7 @@ __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySche
         if (SQ) { accq[0] = zmc_sq_add<F>(accq[0], fa); accq[1] = zmc_sq_add<F>(accq[1], fb); }
     } else {
         zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq);
-        zmc_group_eval<F, SQ>(f, ks, uc, gj, acc + SG, accq + SG);
+        zmc_group_eval<F, SQ>(f, ks, uc, gj, acc + SG, accq + 2);
     }
 }
 
@@ -659,9 +659,10 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
 
         /* lanes stride over the chunk's groups; acc[0..SG) sums the groups at even multiples of 32 from the
          * lane's first one, acc[SG..2SG) those at odd multiples -- whatever UNROLL is, so results do not depend on it */
-        double acc[2 * SG], accq[2 * SG];
+        double acc[2 * SG], accq[4];     /* sums of squares: two accumulators per group in flight are enough */
 #pragma unroll
-        for (int s = 0; s < 2 * SG; ++s) { acc[s] = 0.0; accq[s] = 0.0; }
+        for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
+        accq[0] = accq[1] = accq[2] = accq[3] = 0.0;
         zu32 gi = gb + lane;
         if (ZmcTune<F>::UNROLL == 4) {
             for (; gi + 96u < gfe; gi += 128u) {
@@ -681,7 +682,7 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
                 if ((zu32)s < tail) {
                     const double fv = f.eval(&w[s * D], nullptr);
                     acc[s] = __dadd_rn(acc[s], fv);
-                    if (SQ) accq[s] = zmc_sq_add<F>(accq[s], fv);
+                    if (SQ) accq[s & 1] = zmc_sq_add<F>(accq[s & 1], fv);
                 }
         }
         double sum = acc[0];
@@ -690,9 +691,7 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
         if (SQ) {
-            double sq = accq[0];
-#pragma unroll
-            for (int s = 1; s < 2 * SG; ++s) sq = __dadd_rn(sq, accq[s]);
+            double sq = __dadd_rn(__dadd_rn(accq[0], accq[1]), __dadd_rn(accq[2], accq[3]));
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) sq = __dadd_rn(sq, __shfl_down_sync(0xFFFFFFFFu, sq, off));
             if (lane == 0u) a.partial_q[item] = sq;
