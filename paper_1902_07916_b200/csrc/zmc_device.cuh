@@ -109,6 +109,33 @@ __device__ __forceinline__ void zmc_philox(zu32 c0, zu32 c1, zu32 c2, zu32 c3, c
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+/* The same with the first round's product M0*c0 supplied by the caller: consecutive call indices differ by 1,
+ * so their products differ by M0 -- a 64-bit add on the ALU pipe instead of a multiply on the FMA-heavy pipe. */
+__device__ __forceinline__ void zmc_philox_p0(zu64 p0, zu32 c1, zu32 c2, zu32 c3, const ZmcKeySchedule& ks, zu32* out) {
+    zu32 c0;
+    {
+        const zu64 p1 = (zu64)c2 * (zu64)ZMC_PHILOX_M1;
+        const zu32 n0 = (zu32)(p1 >> 32) ^ c1 ^ ks.k0[0];
+        const zu32 n2 = (zu32)(p0 >> 32) ^ c3 ^ ks.k1[0];
+        c1 = (zu32)p1;
+        c3 = (zu32)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+#pragma unroll
+    for (int r = 1; r < 10; ++r) {
+        const zu64 q0 = (zu64)c0 * (zu64)ZMC_PHILOX_M0;
+        const zu64 q1 = (zu64)c2 * (zu64)ZMC_PHILOX_M1;
+        const zu32 n0 = (zu32)(q1 >> 32) ^ c1 ^ ks.k0[r];
+        const zu32 n2 = (zu32)(q0 >> 32) ^ c3 ^ ks.k1[r];
+        c1 = (zu32)q1;
+        c3 = (zu32)q0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
 /* R3: counter of call q of unit (path P, level l, trial t): (q, t | l<<8 | P[79:64]<<16, P[31:0], P[63:32]) */
 struct ZmcUnitCounter {
     zu32 c1, c2, c3;
@@ -550,7 +577,8 @@ template <int D> struct ZmcGroup {
  * bound by dispatch slots, so what is tuned is the instruction count and the compiler's schedule:
  *   PACKED  evaluate two samples per FFMA2/FADD2/FMUL2 (needs F::HAS_PACKED)
  *   UNROLL  sample groups in flight per lane and loop trip: 2 or 4
- *   MINB    resident CTAs per SM asked of __launch_bounds__ (register cap) */
+ *   MINB    resident CTAs per SM asked of __launch_bounds__ (register cap)
+ *   P0_ADD  first-round products M0*q of a group's later calls by 64-bit addition (ALU pipe) instead of IMAD.WIDE */
 template <class F>
 struct ZmcTune {
     static constexpr int D = F::D;
@@ -558,9 +586,15 @@ struct ZmcTune {
     static constexpr bool PACKED = F::HAS_PACKED && (ZMC_TUNE_PACKED != 0);
     static constexpr int UNROLL = ZMC_TUNE_UNROLL;
     static constexpr int MINB = ZMC_TUNE_MINB;
+#ifdef ZMC_TUNE_P0ADD
+    static constexpr bool P0_ADD = (ZMC_TUNE_P0ADD != 0);
+#else
+    static constexpr bool P0_ADD = false;
+#endif
 #else
     static constexpr bool PACKED = F::HAS_PACKED;
     static constexpr int UNROLL = (D == 4 || D == 6 || D == 12) ? 4 : 2;
+    static constexpr bool P0_ADD = (D == 6);     /* +1 % at D = 6, -1.4 % at D = 9, nil at D = 12 */
     static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && D >= 7) ? 2 : ((D == 4) ? 4 : 3);   /* FP64 at high D spills below 255 registers */
 #endif
 };
@@ -578,8 +612,14 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     zu32 w[4 * CG];
     const zu32 q0 = gi * (zu32)CG;
+    if (ZmcTune<F>::P0_ADD) {      /* one first-round multiply per group, the other calls' products by adding M0 */
+        const zu64 p0 = (zu64)q0 * (zu64)ZMC_PHILOX_M0;
 #pragma unroll
-    for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+        for (int c = 0; c < CG; ++c) zmc_philox_p0(p0 + (zu64)c * (zu64)ZMC_PHILOX_M0, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+    }
     if (ZmcTune<F>::PACKED && SG >= 2) {      /* samples (2i, 2i+1) of the group as one packed evaluation */
 #pragma unroll
         for (int s = 0; s < SG; s += 2) {
