@@ -578,7 +578,9 @@ template <int D> struct ZmcGroup {
  *   PACKED  evaluate two samples per FFMA2/FADD2/FMUL2 (needs F::HAS_PACKED)
  *   UNROLL  sample groups in flight per lane and loop trip: 2 or 4
  *   MINB    resident CTAs per SM asked of __launch_bounds__ (register cap)
- *   P0_ADD  first-round products M0*q of a group's later calls by 64-bit addition (ALU pipe) instead of IMAD.WIDE */
+ *   P0_ADD  first-round products M0*q of a group's later calls by 64-bit addition (ALU pipe) instead of IMAD.WIDE
+ *   P0_CARRY  ... and the group's own first product as a 64-bit induction variable of the sample loop:
+ *           no first-round multiply at all on the FMA-heavy pipe */
 template <class F>
 struct ZmcTune {
     static constexpr int D = F::D;
@@ -588,13 +590,16 @@ struct ZmcTune {
     static constexpr int MINB = ZMC_TUNE_MINB;
 #ifdef ZMC_TUNE_P0ADD
     static constexpr bool P0_ADD = (ZMC_TUNE_P0ADD != 0);
+    static constexpr bool P0_CARRY = (ZMC_TUNE_P0ADD == 2);
 #else
     static constexpr bool P0_ADD = false;
+    static constexpr bool P0_CARRY = false;
 #endif
 #else
     static constexpr bool PACKED = F::HAS_PACKED;
     static constexpr int UNROLL = (D == 4 || D == 6 || D == 12) ? 4 : 2;
-    static constexpr bool P0_ADD = (D == 6);     /* +1 % at D = 6, -1.4 % at D = 9, nil at D = 12 */
+    static constexpr bool P0_ADD = (D == 6 || D == 12);   /* +3.7 % at D = 6, +1.2 % at D = 12, nil at D = 4, -1.5 % at D = 9 */
+    static constexpr bool P0_CARRY = P0_ADD;
     static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && D >= 7) ? 2 : ((D == 4) ? 4 : 3);   /* FP64 at high D spills below 255 registers */
 #endif
 };
@@ -608,12 +613,12 @@ __device__ __forceinline__ double zmc_sq_add(double q, double f) {
 
 template <class F, bool SQ>
 __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
-                                               double* acc, double* accq) {
+                                               double* acc, double* accq, zu64 pg = 0ull, bool have_pg = false) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     zu32 w[4 * CG];
     const zu32 q0 = gi * (zu32)CG;
     if (ZmcTune<F>::P0_ADD) {      /* one first-round multiply per group, the other calls' products by adding M0 */
-        const zu64 p0 = (zu64)q0 * (zu64)ZMC_PHILOX_M0;
+        const zu64 p0 = have_pg ? pg : (zu64)q0 * (zu64)ZMC_PHILOX_M0;
 #pragma unroll
         for (int c = 0; c < CG; ++c) zmc_philox_p0(p0 + (zu64)c * (zu64)ZMC_PHILOX_M0, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
     } else {
@@ -642,22 +647,32 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
 /* groups gi and gj: acc[0..SG) takes gi's samples, acc[SG..2SG) gj's -- the same sums as two zmc_group_eval calls */
 template <class F, bool SQ>
 __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
-                                                    zu32 gj, double* acc, double* accq) {
+                                                    zu32 gj, double* acc, double* accq, zu64 pg = 0ull, bool have_pg = false) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
     if (ZmcTune<F>::PACKED && SG == 1) {      /* one sample per group (D = 4, 8, ..): pack across the two groups */
         zu32 wa[4 * CG], wb[4 * CG];
+        if (ZmcTune<F>::P0_ADD) {
+            const zu64 pa = have_pg ? pg : (zu64)(gi * (zu32)CG) * (zu64)ZMC_PHILOX_M0;
+            const zu64 pb = have_pg ? pg + (zu64)(32 * CG) * (zu64)ZMC_PHILOX_M0 : (zu64)(gj * (zu32)CG) * (zu64)ZMC_PHILOX_M0;
 #pragma unroll
-        for (int c = 0; c < CG; ++c) zmc_philox(gi * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wa[4 * c]);
+            for (int c = 0; c < CG; ++c) zmc_philox_p0(pa + (zu64)c * (zu64)ZMC_PHILOX_M0, uc.c1, uc.c2, uc.c3, ks, &wa[4 * c]);
 #pragma unroll
-        for (int c = 0; c < CG; ++c) zmc_philox(gj * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wb[4 * c]);
+            for (int c = 0; c < CG; ++c) zmc_philox_p0(pb + (zu64)c * (zu64)ZMC_PHILOX_M0, uc.c1, uc.c2, uc.c3, ks, &wb[4 * c]);
+        } else {
+#pragma unroll
+            for (int c = 0; c < CG; ++c) zmc_philox(gi * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wa[4 * c]);
+#pragma unroll
+            for (int c = 0; c < CG; ++c) zmc_philox(gj * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wb[4 * c]);
+        }
         double fa, fb;
         f.eval2(wa, wb, fa, fb);
         acc[0] = __dadd_rn(acc[0], fa);
         acc[1] = __dadd_rn(acc[1], fb);
         if (SQ) { accq[0] = zmc_sq_add<F>(accq[0], fa); accq[1] = zmc_sq_add<F>(accq[1], fb); }
     } else {
-        zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq);
-        zmc_group_eval<F, SQ>(f, ks, uc, gj, acc + SG, accq + 2);
+        /* gj = gi + 32: its first product is gi's plus 32*CG*M0 */
+        zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq, pg, have_pg);
+        zmc_group_eval<F, SQ>(f, ks, uc, gj, acc + SG, accq + 2, pg + (zu64)(32 * CG) * (zu64)ZMC_PHILOX_M0, have_pg);
     }
 }
 
@@ -704,13 +719,19 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
         for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
         accq[0] = accq[1] = accq[2] = accq[3] = 0.0;
         zu32 gi = gb + lane;
+        constexpr bool CARRY = ZmcTune<F>::P0_CARRY;     /* the group's first product as a 64-bit induction variable */
+        zu64 pg = (zu64)(gi * (zu32)CG) * (zu64)ZMC_PHILOX_M0;
         if (ZmcTune<F>::UNROLL == 4) {
             for (; gi + 96u < gfe; gi += 128u) {
-                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq);
-                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi + 64u, gi + 96u, acc, accq);
+                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq, pg, CARRY);
+                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi + 64u, gi + 96u, acc, accq, pg + (zu64)(64 * CG) * (zu64)ZMC_PHILOX_M0, CARRY);
+                pg += (zu64)(128 * CG) * (zu64)ZMC_PHILOX_M0;
             }
         }
-        for (; gi + 32u < gfe; gi += 64u) zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq);
+        for (; gi + 32u < gfe; gi += 64u) {
+            zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq, pg, CARRY);
+            pg += (zu64)(64 * CG) * (zu64)ZMC_PHILOX_M0;
+        }
         if (gi < gfe) zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq);
         if (tail != 0u && ge > full_groups && lane == 0u) {   /* the partial group: only its first `tail` samples exist */
             zu32 w[4 * CG];
