@@ -43,6 +43,8 @@ def workloads():
         "cfg3_gauss9d": W.config3(),
         # BASELINE.json configs[3] with budget 4 per instance (unbudgeted: ~1.7e12 evals)
         "cfg4_batched4d_B4": W.config4().with_(max_groups_per_level=4),
+        # BASELINE.json configs[3] whole, the paper's semantics (about 1.7e12 evaluations, 8e7 level-2 cells, ~5 s)
+        "cfg4_batched4d": W.config4().with_(max_cells_per_level=1024 * 1296 * 96),
         # BASELINE.json configs[4], level 1 only (the 5.2e11 evaluations BASELINE.json quotes)
         "cfg5_sin6d_level1": W.config5(depth=1),
         "cfg1_sin3d_f64": W.config1(),

@@ -163,3 +163,34 @@ def test_fullsize_fast_mode_within_bj_tolerance():
             assert abs(gl.S[c, 1] - S_o) <= tol
         assert abs(v[0] - _closed(w)) <= 4 * sd[0]
         it.close()
+
+
+def test_config4_whole_without_budget():
+    """BASELINE.json configs[3] exactly as given (no budget): 1024 instances, ~6e4 refined cells, ~8e7 level-2 cells,
+    ~1.7e12 evaluations. Too large to dump; checked on what is unique: every instance's integral against its closed form
+    (P4: within 4 sigma), the level bookkeeping (cells = parents * k, evaluations = cells * T * N), no overflow, and the
+    per-instance results of the first instances against budgeted runs whose level 1 is identical."""
+    w = bench.workloads()["cfg4_batched4d"]
+    it = B.from_workload(w, max_cells_per_level=bench.capacity_for(w))
+    it.use_torch_workspace()
+    it.run()
+    v, sd = it.result()
+    st = it.stats()
+    assert st.overflow == 0 and st.nonfinite == 0
+    l1, l2 = st.level[0], st.level[1]
+    assert l1.n_cells == 1024 * w.k and l1.n_refined == l1.n_flagged and l2.n_groups == l1.n_refined
+    assert l2.n_cells == l2.n_groups * w.k and l2.n_refined == 0
+    assert st.total_evals == (l1.n_cells + l2.n_cells) * w.trials * w.n_samples
+    assert 3e4 < l1.n_refined < 1.2e5          # SURVEY 8.0: mean about 62 flagged cells per instance
+    bad = 0
+    zs = []
+    for b in range(w.n_instances):
+        closed = H.closed_exp_quad(w.params[b], w.lower, w.upper)
+        zs.append((v[b] - closed) / sd[b])
+        bad += abs(v[b] - closed) > 4 * sd[b]
+    assert bad == 0
+    zs = np.array(zs)
+    assert abs(zs.mean()) < 0.2 and zs.std() < 1.0      # std overstates the error of the mean (R7), so |z| is well below 1
+    print("cfg4 whole: %d refined, %.3g evals, %.1f ms, z mean %.3f std %.3f" %
+          (l1.n_refined, st.total_evals, st.total_ms, zs.mean(), zs.std()))
+    it.close()
