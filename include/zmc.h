@@ -35,7 +35,7 @@ extern "C" {
 typedef enum zmc_status {
     ZMC_OK = 0,
     ZMC_ERR_ARG = -1,          /* null pointer, non-finite or empty bounds, counts < 1 ... */
-    ZMC_ERR_RANGE = -2,        /* path > 80 bits, g^depth > 2^32, N*D/4 >= 2^32, trials > 255, depth > 15, dim > 16 */
+    ZMC_ERR_RANGE = -2,        /* path > 80 bits, g^depth > 2^32, N*D/4 >= 2^32 - 4096, trials > 255, depth > 15, dim > 16 */
     ZMC_ERR_NO_INTEGRAND = -3, /* zmc_run before zmc_set_integrand* */
     ZMC_ERR_COMPILE = -4,      /* NVRTC failed; the log is in zmc_last_error */
     ZMC_ERR_CUDA = -5,         /* a CUDA runtime call failed (or no device) */

@@ -90,9 +90,9 @@ __device__ __forceinline__ void zmc_plan_level(ZmcLevelInfo& li, zu64 n_groups, 
         if (max_ch < 1) max_ch = 1;
         if (nch > max_ch) nch = max_ch;
     }
-    const zu32 cg = (zu32)((c.sample_groups + nch - 1) / nch);
+    const zu32 cg = (zu32)(((zu64)c.sample_groups + nch - 1) / nch);
     li.chunk_groups = cg;
-    li.n_chunks = (c.sample_groups + cg - 1) / cg;
+    li.n_chunks = (zu32)(((zu64)c.sample_groups + cg - 1) / cg);    /* 64-bit: sample_groups may be within cg of 2^32 */
     li.n_items = units * li.n_chunks;
     li.work_ctr = 0;
     li.n_flagged = 0;

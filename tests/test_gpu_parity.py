@@ -388,3 +388,26 @@ def test_user_integrand_parameter_sweep():
         assert abs(v[b] - H.closed_exp_quad(w.params[b], w.lower, w.upper)) <= 4 * s[b]
     it.close()
     ref.close()
+
+
+def test_maximum_sample_count():
+    """The largest N the counter layout allows (R3: N*D/4 < 2^32 - 4096): D = 1, one cell, N = 2^34 - 2^15 samples per trial,
+    cut into 65536 chunks. Too many for the oracle; the words at the top of the index range are compared bit for bit, and the
+    integral of sin over [0, 3] must come out within 4 sigma at a spread of ~1e-5 (a wrapped or skipped index range would
+    show as a wrong sample count in the estimate's scale)."""
+    N = (1 << 34) - (1 << 15)
+    w = W.Workload("nmax", 1, (0.0,), (3.0,), 1, N, 3, 1, 1.0, 31, W.SIN_SUM, W.F32)
+    with B.from_workload(w, keep_level_stats=True, max_cells_per_level=16) as it:
+        g = it.debug_words(0, 0, 1, 2, N - 64, 64)
+        o = O.unit_words(w.seed, 0, 0, 1, 2, N - 64, 64)
+        np.testing.assert_array_equal(g, o)
+        it.run()
+        v, s = it.result()
+        S = it.level_cells(1).S[0]
+        closed = 1.0 - np.cos(3.0)
+        assert abs(v[0] - closed) <= 4 * s[0] + 1e-7 and s[0] < 2e-5       # 1e-7: the FP32 lattice and zsin's own error
+        # each trial's mean of f is 3 * S / N; three independent estimates agree to a few 1e-5
+        assert np.all(np.abs(3.0 * S / N - closed) < 6e-5)
+    with pytest.raises(B.ZmcError) as e:
+        B.Integrator(1, [0.0], [3.0], 1, 1 << 34, 3, 1, 1.0, 31)
+    assert e.value.status == B.ERR_RANGE
