@@ -411,3 +411,36 @@ def test_maximum_sample_count():
     with pytest.raises(B.ZmcError) as e:
         B.Integrator(1, [0.0], [3.0], 1, 1 << 34, 3, 1, 1.0, 31)
     assert e.value.status == B.ERR_RANGE
+
+
+def test_many_instances():
+    """3000 independent instances with their own keys, parameters, thresholds and budgets (R11): per-instance scans,
+    first/last group bookkeeping and results at a count well above one CTA's width."""
+    rng = np.random.default_rng(3)
+    n = 3000
+    p = np.empty((n, 4))
+    p[:, 0] = 1.0
+    p[:, 1] = (10.0 ** rng.uniform(0, 2, n)).astype(np.float32)
+    p[:, 2:] = (0.2 + 0.6 * rng.random((n, 2))).astype(np.float32)
+    w = W.Workload("many", 2, (0.0, 0.0), (1.0, 1.0), 3, 48, 3, 3, 0.7, 17, W.EXP_QUAD, W.F32, params=p, n_instances=n,
+                   max_groups_per_level=2)
+    it, ores = _run_both(w, max_cells=n * 9 * 4)
+    H.compare_tree(it, ores, w)
+    assert ores.levels[1].n_cells > n * 9 and len(ores.levels) == 3
+    it.close()
+
+
+def test_impossible_size_is_an_error_not_a_crash():
+    """k = 16^10 = 2^40 cells at level 1 passes the range checks but cannot be allocated: zmc_run reports it."""
+    w = W.Workload("huge", 10, (0.0,) * 10, (1.0,) * 10, 16, 4, 2, 1, 1.0, 1, W.SIN_SUM, W.F32)
+    it = B.from_workload(w)
+    with pytest.raises(B.ZmcError) as e:
+        it.run()
+    assert e.value.status in (B.ERR_CUDA, B.ERR_CAPACITY, B.ERR_RANGE)
+    it.close()
+    # and the library still works afterwards
+    w1 = W.config1()
+    it = B.from_workload(w1)
+    it.run()
+    assert abs(it.result()[0][0] - (-4.553120732569151)) < 1e-9
+    it.close()
