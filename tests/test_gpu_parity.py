@@ -444,3 +444,93 @@ def test_impossible_size_is_an_error_not_a_crash():
     it.run()
     assert abs(it.result()[0][0] - (-4.553120732569151)) < 1e-9
     it.close()
+
+
+def test_capacity_boundary_and_grid_independence():
+    """Exactly enough room is enough (5 refined cells of config 1 -> 5 parents); one fewer is an overflow. The result does
+    not depend on the size of the persistent grid (1 CTA, 7 CTAs, the default), bit for bit."""
+    w = W.config1()
+    ref = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 12)
+    ref.run()
+    rv, rs = ref.result()
+    rS = ref.level_cells(2).S
+    for cap, ok in ((5 * 64, True), (4 * 64, False)):
+        it = B.from_workload(w, max_cells_per_level=cap)
+        it.run()
+        if ok:
+            v, s = it.result()
+            assert v[0] == rv[0] and s[0] == rs[0]
+        else:
+            with pytest.raises(B.ZmcError) as e:
+                it.result()
+            assert e.value.status == B.ERR_CAPACITY
+        it.close()
+    for grid in (1, 7):
+        it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 12)
+        it.set_option(B.OPT_GRID_BLOCKS, grid)
+        it.run()
+        v, s = it.result()
+        assert v[0] == rv[0] and s[0] == rs[0] and it.stats().grid_blocks == grid
+        np.testing.assert_array_equal(it.level_cells(2).S, rS)
+        it.close()
+    # a different chunking changes the summation order only
+    it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 12)
+    it.set_option(B.OPT_TARGET_ITEMS, 320)
+    it.run()
+    v, s = it.result()
+    assert abs(v[0] - rv[0]) <= 1e-12 * abs(rv[0]) and np.abs(it.level_cells(2).S - rS).max() <= 1e-12 * w.n_samples
+    it.close()
+    ref.close()
+
+
+def test_api_state_errors_and_context_reuse():
+    w = W.config1()
+    it = B.Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
+    with pytest.raises(B.ZmcError) as e:
+        it.run()
+    assert e.value.status == B.ERR_NO_INTEGRAND
+    with pytest.raises(B.ZmcError) as e:
+        it.workspace_bytes()
+    assert e.value.status == B.ERR_NO_INTEGRAND
+    it.set_integrand(B.SIN_SUM)
+    with pytest.raises(B.ZmcError) as e:
+        it.result()
+    assert e.value.status == B.ERR_NOT_RUN
+    with pytest.raises(B.ZmcError) as e:
+        it.set_integrand(B.EXP_QUAD, np.array([[1.0, 2.0]]), 1)        # too few parameters for D = 3
+    assert e.value.status == B.ERR_ARG
+    with pytest.raises(B.ZmcError) as e:
+        it.set_option(99, 1)
+    assert e.value.status == B.ERR_ARG
+    with pytest.raises(B.ZmcError) as e:
+        it.set_workspace(256, 1 << 20) if False else it.set_workspace(257, 1 << 20)     # not 256-byte aligned
+    assert e.value.status == B.ERR_ARG
+    it.run()
+    a = it.result()
+    with pytest.raises(B.ZmcError) as e:
+        it.level_cells(1)                                              # level stats were not kept
+    assert e.value.status == B.ERR_STATE
+    # the same context, another integrand and instance count
+    p = W.batched_params(4, 3, 9)
+    it.set_integrand(B.EXP_QUAD, p, 4)
+    it.set_option(B.OPT_PRECISION, B.F32)
+    it.run()
+    v, s = it.result()
+    for b in range(4):
+        assert abs(v[b] - H.closed_exp_quad(p[b], w.lower, w.upper)) <= 4 * s[b]
+    # and back: bit-identical to the first run
+    it.set_integrand(B.SIN_SUM)
+    it.set_option(B.OPT_PRECISION, B.F64)
+    it.run()
+    b2 = it.result()
+    assert a[0][0] == b2[0][0] and a[1][0] == b2[1][0]
+    it.close()
+    # a workspace that is too small is refused at run time
+    import torch
+    it = B.from_workload(w)
+    buf = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    it.set_workspace((buf.data_ptr() + 255) & ~255, 1024)
+    with pytest.raises(B.ZmcError) as e:
+        it.run()
+    assert e.value.status == B.ERR_ARG
+    it.close()
