@@ -93,7 +93,10 @@ def compare_tree(it, ores, w: W.Workload, *, tol_sum=1e-12, tol_stat=1e-11, exac
         sc = max(np.abs(ol.mu).max(), ol.s.max(), 1e-300)
         assert np.abs(gl.mu - ol.mu).max() <= tol_stat * sc
         assert np.abs(gl.s - ol.s).max() <= 100 * tol_stat * sc
-        assert np.abs(gl.tau - ol.tau).max() <= 100 * tol_stat * max(ol.tau.max(), 1e-300)
+        # tau = mean(s) + m*pstd(s) is (1 + |m|)-Lipschitz in max|ds|: where s itself is ill-conditioned (cells so small that
+        # f is constant to 9 digits) the thresholds inherit exactly that much and no more
+        ds = float(np.abs(gl.s - ol.s).max())
+        assert np.abs(gl.tau - ol.tau).max() <= 100 * tol_stat * max(ol.tau.max(), 1e-300) + (1.0 + abs(w.sigma_multiplier)) * ds
         if exact_sets:
             np.testing.assert_array_equal(gl.refined, ol.refined)
         n_cmp += ol.n_cells

@@ -534,3 +534,18 @@ def test_api_state_errors_and_context_reuse():
         it.run()
     assert e.value.status == B.ERR_ARG
     it.close()
+
+
+def test_wide_groups_and_maximum_dimension():
+    """k = 60000 cells per sibling group in one dimension (234 compaction tiles per group, integer coordinates up to 3.6e9 at
+    level 2), and D = 16 = ZMC_MAX_DIM with 65536 cells (NVRTC instance, 4 Philox calls per sample)."""
+    w = W.Workload("wide", 1, (-2.0,), (5.0,), 60000, 8, 3, 2, 1.0, 23, W.SIN_SUM, W.F64, max_groups_per_level=3)
+    it, ores = _run_both(w, max_cells=4 * 60000)
+    H.compare_tree(it, ores, w)
+    assert ores.levels[1].n_cells == 3 * 60000
+    it.close()
+    for prec, integrand, params in ((W.F32, W.LINEAR, np.linspace(-1.0, 1.0, 17)[None, :]), (W.F64, W.SIN_SUM, None)):
+        w = W.Workload("d16", 16, (0.0,) * 16, (1.0,) * 16, 2, 9, 3, 1, 1.0, 29, integrand, prec, params=params)
+        it, ores = _run_both(w)
+        H.compare_tree(it, ores, w)
+        it.close()
