@@ -549,3 +549,27 @@ def test_wide_groups_and_maximum_dimension():
         it, ores = _run_both(w)
         H.compare_tree(it, ores, w)
         it.close()
+
+
+def test_two_contexts_on_two_streams():
+    """Distinct contexts are independent: two tree searches enqueued on two streams at the same time, several times over,
+    give the results each gives alone."""
+    import torch
+    wa = W.config2().with_(n_samples=3001, depth=2, max_groups_per_level=2)
+    wb = W.config3().with_(n_samples=1500, depth=3)
+    alone = []
+    for w in (wa, wb):
+        with B.from_workload(w, max_cells_per_level=1 << 17) as it:
+            it.run()
+            alone.append(it.result())
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    ia = B.from_workload(wa, max_cells_per_level=1 << 17)
+    ib = B.from_workload(wb, max_cells_per_level=1 << 17)
+    for _ in range(3):
+        ia.run(sa.cuda_stream)
+        ib.run(sb.cuda_stream)
+        ra, rb = ia.result(), ib.result()
+        assert ra[0][0] == alone[0][0][0] and ra[1][0] == alone[0][1][0]
+        assert rb[0][0] == alone[1][0][0] and rb[1][0] == alone[1][1][0]
+    ia.close()
+    ib.close()
