@@ -85,3 +85,28 @@ def test_no_device_means_error_not_fallback():
         B.Integrator(3, [0.0] * 3, [1.0] * 3, 4, 100, 5, 2, 1.5, 1)
     assert e.value.status == B.ERR_CUDA
     assert B.lib().zmc_microbench(0, None, None, None) == B.ERR_CUDA
+
+
+def test_headline_kernels_keep_their_register_budget():
+    """The sampling kernel's speed hangs on ptxas' schedule (profiles/r1_variants.md: a three-line change once cost 30 registers
+    and 4 %). The build keeps ptxas -v per translation unit: the headline instances must stay within the register count that
+    gives them 4 CTAs per SM, without spills."""
+    from paper_1902_07916_b200 import build as zbuild
+    B.lib()
+    budget = {   # (integrand id, D) of FP32 exact-mode UKEY kernels -> registers for 4 CTAs of 128 threads per SM
+        ("zmc_inst_1_0_2", "ZmcIntegrandILi2ELi6ELi1ELi0EELb1ELb0"): 128,     # sin 6-D: configs 2 and 5
+        ("zmc_inst_1_0_3", "ZmcIntegrandILi3ELi9ELi1ELi0EELb1ELb0"): 128,     # Gaussian 9-D: config 3
+        ("zmc_inst_1_0_3", "ZmcIntegrandILi3ELi12ELi1ELi0EELb1ELb0"): 128,    # Gaussian 12-D: paper Table 4
+        ("zmc_inst_1_0_3", "ZmcIntegrandILi3ELi4ELi1ELi0EELb0ELb0"): 102,     # Gaussian 4-D, per-item key: config 4 (5 CTAs)
+    }
+    for (unit, key), limit in budget.items():
+        path = os.path.join(zbuild.OBJ, unit + ".ptxas.txt")
+        if not os.path.exists(path):
+            pytest.skip("no ptxas log (library not built here)")
+        lines = open(path).read().splitlines()
+        idx = [i for i, l in enumerate(lines) if "Compiling entry function" in l and "zmc_sample_kernel" in l and key in l]
+        assert len(idx) == 1, (unit, key, len(idx))
+        block = " ".join(lines[idx[0]: idx[0] + 4])
+        regs = int(re.search(r"Used (\d+) registers", block).group(1))
+        assert regs <= limit, (key, regs, limit)
+        assert "0 bytes spill stores" in block, block
