@@ -236,10 +236,16 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
-    torch.cuda.set_device(local_rank)
+    n_dev = torch.cuda.device_count()
+    shared = int(os.environ.get("LOCAL_WORLD_SIZE", world)) > n_dev   # more ranks than GPUs (a smoke run of the N > 1 path on one GPU):
+    local_dev = local_rank % n_dev                      # the ranks share devices; NCCL cannot, so the plumbing goes over gloo
+    torch.cuda.set_device(local_dev)
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if shared or os.environ.get("ZMC_BENCH_BACKEND") == "gloo":
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_dev))
     math = B.MATH_EXACT if args.math == "exact" else B.MATH_FAST
     w_rank = w.with_(seed=w.seed + rank)            # replicas differ only in the seed
     cap = capacity_for(w)
@@ -247,7 +253,7 @@ def main():
     order = B.BUDGET_LARGEST_SPREAD if args.budget_order == "spread" else B.BUDGET_PATH_ORDER
     it = B.from_workload(w_rank, math=math, max_cells_per_level=cap, use_graph=args.graph, spread=spread, budget_order=order)
     it.use_torch_workspace()
-    props = torch.cuda.get_device_properties(local_rank)
+    props = torch.cuda.get_device_properties(local_dev)
     n_sm = props.multi_processor_count
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
@@ -262,7 +268,7 @@ def main():
         it.run(stream.cuda_stream)
     it.result()
     barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    sampler = ClockSampler(local_dev) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     t_wall = time.perf_counter()
