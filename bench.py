@@ -56,6 +56,18 @@ def workloads():
     }
 
 
+# what each bench workload leaves out of (or adds to) the BASELINE.json config it is named after, stated in the JSON line
+DEVIATIONS = {
+    "cfg2_sin6d_depth3_B16": "BASELINE.json configs[1] at its full depth 3 with a refinement budget of 16 cells per level (DESIGN.md R12): "
+                             "under the paper's rule m = 1.5 flags ~8 % of the cells by chance and depth 3 needs ~2.2e14 evaluations (~14 min); "
+                             "cfg2_sin6d_depth2 is the same config without budget, cut at depth 2",
+    "cfg2_sin6d_depth2": "BASELINE.json configs[1] under the paper's rule (no budget), depth 2 of 3",
+    "cfg2_sin6d_depth1": "BASELINE.json configs[1], level 1 only",
+    "cfg4_batched4d_B4": "BASELINE.json configs[3] with a refinement budget of 4 cells per instance; cfg4_batched4d is the config as given",
+    "cfg5_sin6d_level1": "BASELINE.json configs[4], level 1 only (the 5.24e11 evaluations it quotes); deeper levels need > 2e16 evaluations",
+}
+
+
 def capacity_for(w):
     """max_cells_per_level the bench (and the full-size parity tests) run a workload with: what its budget
     or depth bounds, else 0 = the library's automatic capacity."""
@@ -318,7 +330,8 @@ def main():
                        "trials": w.trials, "depth": w.depth, "sigma_multiplier": w.sigma_multiplier, "seed": w.seed,
                        "n_instances": w.n_instances, "max_groups_per_level": w.max_groups_per_level, "math": args.math, "graph": bool(args.graph), "spread": args.spread, "budget_order": args.budget_order,
                        "evals_per_step": evals_step, "l2": "256 MiB buffer written between steps (flush); the path reads ~16 B per cell",
-                       "parallelism": "replicas x%d" % world},
+                       "parallelism": "replicas x%d" % world,
+                       "deviation": DEVIATIONS.get(args.workload)},
             "result": {"value": float(value_v[0]), "std": float(value_s[0])},
             "wall_ms_per_step": 1e3 * t_wall / args.steps,
             "gpu_launches": launches_per_step(w.depth, order == B.BUDGET_LARGEST_SPREAD and w.max_groups_per_level > 0) * args.steps,
