@@ -135,3 +135,75 @@ def test_fullsize_sample_spread_and_largest_spread_budget():
     print("cfg2 with R13+R14: value %.6f +- %.4f, z = %.2f" % (v[0], sd[0], z))
     assert abs(z) < 4.0
     it.close()
+
+
+def test_largest_spread_budget_with_exact_ties():
+    """R14's tie rule (equal spreads are taken in ascending path order) cannot be reached with the built-in integrands: their
+    spreads never coincide. A user integrand with two values -- stripes of width 1/37 in x0, N = 1, T = 2 -- makes every cell's
+    spread exactly 0 or V/2, so dozens of flagged cells tie at the pivot. Checked against the brute-force selection in numpy
+    (tests/helpers.py host_control) from the dumped (mu, s): pivot, quota and the path-order ranks among the ties."""
+    src = r"""
+    __device__ double stripes(const double* x, int dim, const double* p, int np) { return (double)(((int)(x[0] * 37.0)) & 1); }
+    __device__ float stripes(const float* x, int dim, const float* p, int np) { return (float)(((int)(x[0] * 37.0f)) & 1); }
+    """
+    k, B_ = 64, 5
+    it = B.Integrator(2, [0.0, 0.0], [1.0, 1.0], 8, 1, 2, 3, 0.0, 41)
+    it.set_integrand_source(src, "stripes", None, 1)
+    it.set_option(B.OPT_MAX_GROUPS_PER_LEVEL, B_)
+    it.set_option(B.OPT_BUDGET_ORDER, B.BUDGET_LARGEST_SPREAD)
+    it.set_option(B.OPT_KEEP_LEVEL_STATS, 1)
+    it.set_option(B.OPT_MAX_CELLS_PER_LEVEL, 1 << 12)
+    it.run()
+    v, s = it.result()
+    parents = None
+    tied_levels = 0
+    for level in (1, 2, 3):
+        gl = it.level_cells(level)
+        n = len(gl.mu)
+        assert n == (1 if level == 1 else B_) * k
+        if parents is not None:
+            assert gl.path == [p * k + j for p in parents for j in range(k)]
+        V = (1.0 / 8 ** level) ** 2
+        assert set(np.unique(gl.s)) <= {0.0, V / 2}                     # exact ties by construction
+        tau_c, refined, lv, lvar = H.host_control(gl.mu, gl.s, k, level, 3, 0.0, np.zeros(n, dtype=np.int64), budget=B_,
+                                                  largest_spread=True)
+        flagged = gl.s > tau_c
+        if level < 3:
+            assert flagged.sum() > B_ and np.all(gl.s[flagged] == V / 2)
+            tied_levels += 1
+            assert list(np.nonzero(refined)[0]) == list(np.nonzero(flagged)[0][:B_])      # ties: first in path order
+        np.testing.assert_array_equal(gl.refined.astype(bool), refined)
+        parents = [gl.path[i] for i in np.nonzero(refined)[0]]
+    assert tied_levels == 2
+    it.close()
+
+
+def test_largest_spread_budget_with_ties_below_larger_spreads():
+    """As above with a three-valued integrand (0, 1, 3 in stripes): spreads are 0, V/2, V or 3V/2, so the pivot's ties sit below
+    strictly larger spreads and only part of them fits the budget (quota < number of ties)."""
+    src = r"""
+    __device__ double steps(const double* x, int dim, const double* p, int np) { const int j = ((int)(x[0] * 53.0)) % 3; return j == 2 ? 3.0 : (double)j; }
+    __device__ float steps(const float* x, int dim, const float* p, int np) { const int j = ((int)(x[0] * 53.0f)) % 3; return j == 2 ? 3.0f : (float)j; }
+    """
+    k, B_ = 64, 26      # this seed: 21 cells at 3V/2, then the ties at V
+    it = B.Integrator(2, [0.0, 0.0], [1.0, 1.0], 8, 1, 2, 2, 0.0, 43)
+    it.set_integrand_source(src, "steps", None, 1)
+    it.set_option(B.OPT_MAX_GROUPS_PER_LEVEL, B_)
+    it.set_option(B.OPT_BUDGET_ORDER, B.BUDGET_LARGEST_SPREAD)
+    it.set_option(B.OPT_KEEP_LEVEL_STATS, 1)
+    it.set_option(B.OPT_MAX_CELLS_PER_LEVEL, 1 << 12)
+    it.run()
+    it.result()
+    gl = it.level_cells(1)
+    V = 1.0 / 64
+    assert set(np.unique(gl.s)) <= {0.0, V / 2, V, 1.5 * V}
+    tau_c, refined, _, _ = H.host_control(gl.mu, gl.s, k, 1, 2, 0.0, np.zeros(k, dtype=np.int64), budget=B_, largest_spread=True)
+    flagged = gl.s > tau_c
+    order = sorted(np.nonzero(flagged)[0], key=lambda i: (-gl.s[i], i))
+    pivot = gl.s[order[B_ - 1]]
+    n_greater = int(np.sum(gl.s[flagged] > pivot))
+    n_ties = int(np.sum(gl.s[flagged] == pivot))
+    assert 0 < n_greater < B_ and n_ties > B_ - n_greater, (n_greater, n_ties)        # the case the quota exists for
+    np.testing.assert_array_equal(gl.refined.astype(bool), refined)
+    assert it.level_cells(2).path == [int(p) * k + j for p in np.nonzero(refined)[0] for j in range(k)]
+    it.close()
