@@ -118,7 +118,10 @@ int zmc_set_workspace(zmc_ctx* ctx, void* workspace, size_t bytes);
 
 /* Enqueue the whole tree search -- every level's sampling, statistics, threshold, flag and compaction
  * kernels -- on cuda_stream (a cudaStream_t; NULL = the default stream) and return without
- * synchronising. No host decision is taken between levels. */
+ * synchronising. No host decision is taken between levels.
+ * The first zmc_run after zmc_set_integrand* or a layout change does the one-time work first: kernel
+ * selection (NVRTC if needed), workspace allocation, parameter upload and key derivation, and waits
+ * for that upload (the derived key of a single-instance run travels back as a launch parameter). */
 int zmc_run(zmc_ctx* ctx, void* cuda_stream);
 
 /* Synchronise the run's stream and fetch, per instance, the integral estimate (sum of accepted cell
