@@ -194,3 +194,30 @@ def test_config4_whole_without_budget():
     print("cfg4 whole: %d refined, %.3g evals, %.1f ms, z mean %.3f std %.3f" %
           (l1.n_refined, st.total_evals, st.total_ms, zs.mean(), zs.std()))
     it.close()
+
+
+def test_zscore_calibration_at_bench_size():
+    """The estimator's sampling distribution at BASELINE.json configs[1]'s full level-1 size (4096 cells x 5 trials x 1e5 samples,
+    2e9 evaluations per run), 120 seeds per mode -- a check no CPU can do and one that sees every sample the kernel draws:
+      R13 (spread from the samples): z = (value - closed)/std is N(0, 1);
+      R5/R7 (the paper's reading): the same z has variance 1/(T-1) -- std overstates the error of the mean by sqrt(T-1),
+      as DESIGN.md R7 says -- and the two modes return the same value (the spread does not enter mu)."""
+    base = bench.workloads()["cfg2_sin6d_depth1"]
+    closed = H.closed_sin_sum(base.lower, base.upper)
+    n = 120
+    z = {B.SPREAD_SAMPLES: [], B.SPREAD_TRIALS: []}
+    vals = {B.SPREAD_SAMPLES: [], B.SPREAD_TRIALS: []}
+    for seed in range(n):
+        w = base.with_(seed=5000 + seed)
+        for spread in z:
+            with B.from_workload(w, max_cells_per_level=w.k, spread=spread) as it:
+                it.run()
+                v, s = it.result()
+            z[spread].append((v[0] - closed) / s[0])
+            vals[spread].append(v[0])
+    assert vals[B.SPREAD_SAMPLES] == vals[B.SPREAD_TRIALS]
+    zs, zt = np.array(z[B.SPREAD_SAMPLES]), np.array(z[B.SPREAD_TRIALS])
+    print("z (samples): mean %.3f var %.3f ; z (trials): mean %.3f var %.3f (1/(T-1) = %.3f)" %
+          (zs.mean(), zs.var(), zt.mean(), zt.var(), 1.0 / (base.trials - 1)))
+    assert abs(zs.mean()) < 3.5 / math.sqrt(n) and 0.70 < zs.var() < 1.40
+    assert 0.70 / (base.trials - 1) < zt.var() < 1.40 / (base.trials - 1)
