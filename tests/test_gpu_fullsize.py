@@ -221,3 +221,33 @@ def test_zscore_calibration_at_bench_size():
           (zs.mean(), zs.var(), zt.mean(), zt.var(), 1.0 / (base.trials - 1)))
     assert abs(zs.mean()) < 3.5 / math.sqrt(n) and 0.70 < zs.var() < 1.40
     assert 0.70 / (base.trials - 1) < zt.var() < 1.40 / (base.trials - 1)
+
+
+def test_gaussian_tree_is_unbiased_over_seeds():
+    """BASELINE.json configs[2] whole (depth 4, refinement homing in on the peak), 60 seeds per mode: the mean of the results
+    is 1 within 4 standard errors of that mean (no bias from R9's extended range, the refinement or the compaction), the
+    reported std brackets the observed scatter (R13: about equal; the paper's reading: about sqrt(T-1) larger), and every
+    run refines exactly the centre cell at levels 1-3."""
+    base = bench.workloads()["cfg3_gauss9d"]
+    out = {}
+    for spread in (B.SPREAD_SAMPLES, B.SPREAD_TRIALS):
+        vals, sds = [], []
+        for seed in range(60):
+            w = base.with_(seed=7000 + seed)
+            with B.from_workload(w, max_cells_per_level=bench.capacity_for(w), spread=spread) as it:
+                it.run()
+                v, s = it.result()
+                st = it.stats()
+            assert [st.level[l].n_refined for l in range(4)] == [1, 1, 1, 0]
+            vals.append(v[0])
+            sds.append(s[0])
+        out[spread] = (np.array(vals), np.array(sds))
+    vs, ss = out[B.SPREAD_SAMPLES]
+    vt, st_ = out[B.SPREAD_TRIALS]
+    assert np.array_equal(vs, vt)
+    scatter = vs.std(ddof=1)
+    assert abs(vs.mean() - 1.0) < 4 * scatter / math.sqrt(len(vs))
+    assert 0.8 * scatter < ss.mean() < 1.6 * scatter                   # R13: a 1-sigma error (slightly conservative here)
+    assert 1.5 * scatter < st_.mean() < 3.5 * scatter                  # paper reading: ~sqrt(T-1) = 2 times the scatter
+    print("cfg3 over 60 seeds: mean %.6f, scatter %.6f, reported std R13 %.6f, paper reading %.6f" %
+          (vs.mean(), scatter, ss.mean(), st_.mean()))
