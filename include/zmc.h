@@ -104,7 +104,9 @@ int zmc_set_integrand(zmc_ctx* ctx, int builtin_id, const double* params, int pa
  * zmc_run is called,
  *     __device__ float  fn_name(const float*  x, int dim, const float*  p, int np)   (ZMC_F32)
  *     __device__ double fn_name(const double* x, int dim, const double* p, int np)   (ZMC_F64)
- * x = the sample point, p = this instance's parameters. Parity with a CPU holds for built-ins only. */
+ * x = the sample point, p = this instance's parameters. Parity with a CPU holds for built-ins only.
+ * Compiled programs are cached per process, and on disk as well if the environment variable ZMC_CACHE_DIR names a
+ * writable directory (keyed by the complete program text; a stale or foreign file is ignored). */
 int zmc_set_integrand_source(zmc_ctx* ctx, const char* cuda_src, const char* fn_name, const double* params,
                              int params_per_instance, int n_instances);
 
@@ -147,6 +149,8 @@ typedef struct zmc_stats_t {
     float total_ms;                 /* first kernel to last kernel of the run */
     int32_t regs_per_thread;        /* sampling kernel */
     int32_t grid_blocks, block_threads;
+    int32_t kernel_origin;          /* sampling kernel: 0 pre-compiled, 1 compiled by NVRTC for this context, 2 from the process-wide
+                                       cache, 3 from the on-disk cache (ZMC_CACHE_DIR) */
     zmc_level_stats level[ZMC_MAX_DEPTH];
 } zmc_stats_t;
 
