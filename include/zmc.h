@@ -185,8 +185,8 @@ int zmc_debug_points(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t
                      const uint32_t* coords, int trial, uint64_t n, double* x, double* f);
 
 /* Issue-rate microbenchmarks of the pipes the path uses (roofline denominator).
- * which: 0 IMAD.WIDE.U32, 1 LOP3, 2 IMAD.WIDE+LOP3 (Philox round mix), 3 FFMA, 4 FADD, 5 DADD, 6 F2F.F64.F32,
- *        7 MUFU.SIN, 8 MUFU.EX2, 9 DFMA, 10 Philox4x32-10 calls, 11 I2F.F64.U32, 12 LEA.HI,
+ * which: 0 IMAD.WIDE.U32, 1 LOP3, 2 IMAD.WIDE+LOP3 (Philox round mix), 3 FFMA, 4 FADD, 5 DADD, 6 F2F.F64.F32 + F2F.F32.F64 (pair),
+ *        7 MUFU.SIN, 8 MUFU.EX2, 9 DFMA, 10 Philox4x32-10 calls, 11 I2F.F64.U32 + F2I.U32.F64 (pair), 12 LEA.HI,
  *        13 IMAD (lo), 14 IMAD.HI.U32, 15 64-bit add (IADD3 + IADD3.X, counted as one), 16 IMAD.WIDE.U32 by a register
  *        100 + 10*X + j: Philox4x32-10 calls, each followed by K = {0, 10, 20, 40}[j] extra independent instructions of
  *        kind X = 1 LOP3, 2 FFMA, 3 FADD, 4 DADD, 5 FFMA2, 6 IMAD, 7 SHF (the cost of an instruction next to the generator)

@@ -59,22 +59,16 @@ __global__ void __launch_bounds__(256, 4) mb_kernel(zu32* sink, unsigned long lo
                 asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(fc));
             } else if (WHICH == 5) {     /* DADD */
                 asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(d[i]) : "d"(dc));
-            } else if (WHICH == 6) {     /* F2F.F64.F32 (+ F2F.F32.F64 back would double count: use a float source chain) */
-                double t;
-                asm volatile("cvt.f64.f32 %0, %1;" : "=d"(t) : "f"(f[i]));
-                d[i] = t;
-                asm volatile("" : "+f"(f[i]));
+            } else if (WHICH == 6) {     /* F2F.F64.F32 + F2F.F32.F64 as a dependent pair (one alone is hoisted by the compiler) */
+                asm volatile("{ .reg .f64 t; cvt.f64.f32 t, %0; cvt.rn.f32.f64 %0, t; }" : "+f"(f[i]));
             } else if (WHICH == 7) {     /* MUFU.SIN */
                 asm volatile("sin.approx.ftz.f32 %0, %0;" : "+f"(f[i]));
             } else if (WHICH == 8) {     /* MUFU.EX2 */
                 asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(f[i]));
             } else if (WHICH == 9) {     /* DFMA */
                 asm volatile("fma.rn.f64 %0, %0, %1, %1;" : "+d"(d[i]) : "d"(dc));
-            } else if (WHICH == 11) {    /* I2F.F64.U32 */
-                double t;
-                asm volatile("cvt.rn.f64.u32 %0, %1;" : "=d"(t) : "r"(r[i]));
-                d[i] = t;
-                asm volatile("" : "+r"(r[i]));
+            } else if (WHICH == 11) {    /* I2F.F64.U32 + F2I.U32.F64 as a dependent pair */
+                asm volatile("{ .reg .f64 t; cvt.rn.f64.u32 t, %0; cvt.rzi.u32.f64 %0, t; }" : "+r"(r[i]));
             } else if (WHICH == 12) {    /* LEA.HI-like: (w >> 9) | 0x3F800000 */
                 asm volatile("{ .reg .b32 t; shr.u32 t, %0, 9; or.b32 %0, t, 0x3F800000; }" : "+r"(r[i]));
             } else if (WHICH == 13) {    /* IMAD (low 32 bits of a 32x32 product, plus an addend) */
@@ -255,7 +249,7 @@ extern "C" int zmc_microbench(int which, void* stream, double* per_sm_clk, doubl
     if (e != cudaSuccess) return e == cudaErrorInvalidValue ? ZMC_ERR_ARG : ZMC_ERR_CUDA;
     /* per thread: kIters * kIlp instructions (which 2: 2 each ; which 10: kIlp/2 Philox calls per step) */
     double per_thread = (double)kIters * kIlp;
-    if (which == 2) per_thread *= 2.0;
+    if (which == 2 || which == 6 || which == 11) per_thread *= 2.0;
     if (which == 10) per_thread = (double)kIters * (kIlp / 2);
     if (which >= 100) per_thread = (double)(kIters / 4) * 4.0;   /* Philox calls */
     const double warps_per_sm = 4.0 * 256.0 / 32.0;

@@ -8,13 +8,9 @@ for IMAD.WIDE.U32, LOP3, FFMA, ... and whole Philox4x32-10 calls.
 from . import binding as B
 
 NAMES = {0: "IMAD.WIDE.U32", 1: "LOP3", 2: "IMAD.WIDE.U32 + LOP3 (Philox round mix)", 3: "FFMA", 4: "FADD", 5: "DADD",
-         7: "MUFU.SIN", 8: "MUFU.EX2", 9: "DFMA", 10: "Philox4x32-10 calls (x32 lanes)",
-         12: "LEA.HI-like (shr + or)", 13: "IMAD.U32 lo", 14: "IMAD.HI.U32",
+         6: "F2F.F64.F32 + F2F.F32.F64 (dependent pair, per instruction)", 7: "MUFU.SIN", 8: "MUFU.EX2", 9: "DFMA", 10: "Philox4x32-10 calls (x32 lanes)",
+         11: "I2F.F64.U32 + F2I.U32.F64 (dependent pair, per instruction)", 12: "LEA.HI-like (shr + or)", 13: "IMAD.U32 lo", 14: "IMAD.HI.U32",
          15: "IADD3 + IADD3.X (64-bit add)", 16: "IMAD.WIDE.U32 with register multiplier"}
-
-
-# which = 6 (F2F.F64.F32) and 11 (I2F.F64.U32) exist in the library but are not listed: the compiler hoists the
-# conversion out of the timing loop, so they measure nothing.
 
 
 def main():
