@@ -110,3 +110,35 @@ def test_headline_kernels_keep_their_register_budget():
         regs = int(re.search(r"Used (\d+) registers", block).group(1))
         assert regs <= limit, (key, regs, limit)
         assert "0 bytes spill stores" in block, block
+
+
+def test_binding_constants_match_the_header():
+    """Every enumerator of include/zmc.h that the ctypes binding mirrors has the same value there, and the ctypes
+    structures have the size the C compiler gives them."""
+    text = open(os.path.join(ROOT, "include", "zmc.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    enums = {k: int(v) for k, v in re.findall(r"\b(ZMC_[A-Z0-9_]+)\s*=\s*(-?\d+)", text)}
+    mirror = {
+        "ZMC_OK": B.OK, "ZMC_ERR_ARG": B.ERR_ARG, "ZMC_ERR_RANGE": B.ERR_RANGE, "ZMC_ERR_NO_INTEGRAND": B.ERR_NO_INTEGRAND,
+        "ZMC_ERR_COMPILE": B.ERR_COMPILE, "ZMC_ERR_CUDA": B.ERR_CUDA, "ZMC_ERR_CAPACITY": B.ERR_CAPACITY,
+        "ZMC_ERR_NOT_RUN": B.ERR_NOT_RUN, "ZMC_ERR_STATE": B.ERR_STATE,
+        "ZMC_CONST": B.CONST, "ZMC_LINEAR": B.LINEAR, "ZMC_SIN_SUM": B.SIN_SUM, "ZMC_EXP_QUAD": B.EXP_QUAD, "ZMC_USER": B.USER,
+        "ZMC_OPT_PRECISION": B.OPT_PRECISION, "ZMC_OPT_MATH": B.OPT_MATH, "ZMC_OPT_MAX_GROUPS_PER_LEVEL": B.OPT_MAX_GROUPS_PER_LEVEL,
+        "ZMC_OPT_KEEP_LEVEL_STATS": B.OPT_KEEP_LEVEL_STATS, "ZMC_OPT_MAX_CELLS_PER_LEVEL": B.OPT_MAX_CELLS_PER_LEVEL,
+        "ZMC_OPT_GRID_BLOCKS": B.OPT_GRID_BLOCKS, "ZMC_OPT_TARGET_ITEMS": B.OPT_TARGET_ITEMS, "ZMC_OPT_USE_GRAPH": B.OPT_USE_GRAPH,
+        "ZMC_OPT_SPREAD": B.OPT_SPREAD, "ZMC_OPT_BUDGET_ORDER": B.OPT_BUDGET_ORDER,
+        "ZMC_F64": B.F64, "ZMC_F32": B.F32, "ZMC_MATH_EXACT": B.MATH_EXACT, "ZMC_MATH_FAST": B.MATH_FAST,
+        "ZMC_SPREAD_TRIALS": B.SPREAD_TRIALS, "ZMC_SPREAD_SAMPLES": B.SPREAD_SAMPLES,
+        "ZMC_BUDGET_PATH_ORDER": B.BUDGET_PATH_ORDER, "ZMC_BUDGET_LARGEST_SPREAD": B.BUDGET_LARGEST_SPREAD,
+    }
+    for name, value in mirror.items():
+        assert enums[name] == value, name
+    assert int(re.search(r"#define ZMC_MAX_DEPTH (\d+)", text).group(1)) == B.MAX_DEPTH
+    # struct sizes as the C compiler sees them
+    src = '#include <stdio.h>\n#include "zmc.h"\nint main(void) { printf("%zu %zu\\n", sizeof(zmc_level_stats), sizeof(zmc_stats_t)); return 0; }\n'
+    import tempfile
+    with tempfile.TemporaryDirectory() as d:
+        open(os.path.join(d, "s.c"), "w").write(src)
+        subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), "-o", os.path.join(d, "s"), os.path.join(d, "s.c")], check=True)
+        a, b = subprocess.run([os.path.join(d, "s")], capture_output=True, text=True, check=True).stdout.split()
+    assert int(a) == C.sizeof(B.LevelStats) and int(b) == C.sizeof(B.Stats)
