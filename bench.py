@@ -188,6 +188,31 @@ def oracle_sample(w, n_units, seed_offset=0):
     return n_units * w.n_samples, dt
 
 
+def _oracle_worker(job):
+    """One process of the all-cores oracle baseline (spawned before CUDA is touched)."""
+    name, precision, units, offset = job
+    w = workloads()[name]
+    if precision != "workload":
+        w = w.with_(precision=precision)
+    ev, sec = oracle_sample(w, units, offset)
+    return ev, sec
+
+
+def oracle_all_cores(name, precision, units_per_core):
+    """The oracle, as it stands, in one process per host core (it is single-threaded): aggregate evaluations/s."""
+    import concurrent.futures as cf
+    import multiprocessing as mp
+    cores = os.cpu_count() or 1
+    t0 = time.perf_counter()
+    with cf.ProcessPoolExecutor(max_workers=cores, mp_context=mp.get_context("spawn")) as ex:
+        res = list(ex.map(_oracle_worker, [(name, precision, units_per_core, 1000 + i) for i in range(cores)]))
+    wall = time.perf_counter() - t0
+    ev = sum(e for e, _ in res)
+    busy = max(s for _, s in res)
+    return {"value": ev / busy, "unit": UNIT, "cores": cores, "kind": "oracle, one process per core",
+            "sample": "%d (cell,trial) units per core, %.1f s busy, %.1f s wall with process start-up" % (units_per_core, busy, wall)}
+
+
 def run_reference(args, w, name):
     """--impl reference: the oracle on the host cores, same metric/config; each step a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -226,6 +251,7 @@ def main():
     ap.add_argument("--budget-order", default="path", choices=["path", "spread"], help="DESIGN.md R14")
     ap.add_argument("--graph", action="store_true", help="replay each step as one CUDA graph (ZMC_OPT_USE_GRAPH)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle in one process per host core (extra key)")
     ap.add_argument("--no-extra", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
@@ -238,6 +264,9 @@ def main():
     if args.impl == "reference":
         run_reference(args, w, args.workload)
         return
+    all_cores = None
+    if args.cpu_all_cores and int(os.environ.get("RANK", "0")) == 0:      # before CUDA is initialised in this process
+        all_cores = oracle_all_cores(args.workload, args.precision, max(1, int(1.0e8 // w.n_samples)))
 
     import numpy as np
     import torch
@@ -394,6 +423,8 @@ def main():
             line["cpu_baseline"] = {"value": ev_c / sec_c, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": "%d (cell,trial) units of level 1 of %s, %d samples each, single thread, %.1f s" %
                                               (units, args.workload, w.n_samples, sec_c)}
+        if all_cores is not None:
+            line["cpu_baseline_all_cores"] = all_cores
         print(json.dumps(line), flush=True)
     it.close()
     if world > 1:
