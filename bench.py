@@ -47,6 +47,9 @@ def workloads():
         "cfg4_batched4d": W.config4().with_(max_cells_per_level=1024 * 1296 * 96),
         # BASELINE.json configs[4], level 1 only (the 5.2e11 evaluations BASELINE.json quotes)
         "cfg5_sin6d_level1": W.config5(depth=1),
+        # BASELINE.json configs[4] to its full depth 4 as SURVEY R12 prescribes: level 1 is the whole 262144-cell group (~4e4 cells
+        # flagged), the budget keeps one cell per level, so levels 2-4 are three more 262144-cell groups (2.1e12 evaluations, ~8 s)
+        "cfg5_sin6d_depth4_B1": W.config5(depth=4, budget=1),
         "cfg1_sin3d_f64": W.config1(),
         # the paper's 12-D Gaussian (Table 4: 47.6 s on one V100), paper's own sizes
         "cfg12_gauss12d": W.gauss12d(),
@@ -64,6 +67,8 @@ DEVIATIONS = {
     "cfg2_sin6d_depth2": "BASELINE.json configs[1] under the paper's rule (no budget), depth 2 of 3",
     "cfg2_sin6d_depth1": "BASELINE.json configs[1], level 1 only",
     "cfg4_batched4d_B4": "BASELINE.json configs[3] with a refinement budget of 4 cells per instance; cfg4_batched4d is the config as given",
+    "cfg5_sin6d_depth4_B1": "BASELINE.json configs[4] at its full depth 4 with a refinement budget of 1 cell per level (DESIGN.md R12): level 1 flags "
+                            "~4e4 of its 262144 cells, the compaction keeps the first; without budget level 2 alone needs > 2e16 evaluations",
     "cfg5_sin6d_level1": "BASELINE.json configs[4], level 1 only (the 5.24e11 evaluations it quotes); deeper levels need > 2e16 evaluations",
 }
 
@@ -251,7 +256,7 @@ def main():
     ap.add_argument("--budget-order", default="path", choices=["path", "spread"], help="DESIGN.md R14")
     ap.add_argument("--graph", action="store_true", help="replay each step as one CUDA graph (ZMC_OPT_USE_GRAPH)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle in one process per host core (extra key)")
+    ap.add_argument("--no-cpu-all-cores", action="store_true", help="skip the oracle-on-every-host-core baseline (cpu_baseline_all_cores)")
     ap.add_argument("--no-extra", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
@@ -265,7 +270,8 @@ def main():
         run_reference(args, w, args.workload)
         return
     all_cores = None
-    if args.cpu_all_cores and int(os.environ.get("RANK", "0")) == 0:      # before CUDA is initialised in this process
+    if (not args.no_cpu_all_cores and not args.no_cpu_baseline and int(os.environ.get("RANK", "0")) == 0
+            and int(os.environ.get("WORLD_SIZE", "1")) == 1):      # before CUDA is initialised in this process
         all_cores = oracle_all_cores(args.workload, args.precision, max(1, int(1.0e8 // w.n_samples)))
 
     import numpy as np
@@ -388,19 +394,31 @@ def main():
                        "d2h_bytes_per_step": 16 * w.n_instances + 4, "ms_per_step": 1e3 * dt / e2e_steps,
                        "what": "zmc_create + zmc_set_integrand + zmc_set_option + zmc_set_workspace + zmc_run + zmc_result + zmc_destroy per step, host arrays in, host doubles out"}
 
-        if world == 1 and not args.no_extra and args.workload != "cfg3_gauss9d":
-            # time-to-result of the 9-D workload (BASELINE.json metric: "time-to-result at 6-D and 9-D")
-            w3 = wl["cfg3_gauss9d"]
-            it3 = B.from_workload(w3, math=math, max_cells_per_level=capacity_for(w3))
-            for _ in range(3):
-                it3.run(stream.cuda_stream)
-            v3, s3 = it3.result()
-            st3 = it3.stats()
-            line["time_to_result"] = {args.workload: {"ms": ms_per_step, "value": float(value_v[0]), "std": float(value_s[0])},
-                                      "cfg3_gauss9d": {"ms": st3.total_ms, "value": float(v3[0]), "std": float(s3[0]),
-                                                       "evals": int(st3.total_evals),
-                                                       "evals_per_s": st3.total_evals / (st3.total_ms * 1e-3)}}
-            it3.close()
+        if world == 1 and not args.no_extra:
+            # BASELINE.json metric: "time-to-result at 6-D and 9-D" -- one whole tree search each, device time from zmc_stats
+            # (first kernel to last kernel), after one untimed run of the same context
+            line["time_to_result"] = {args.workload: {"ms": ms_per_step, "value": float(value_v[0]), "std": float(value_s[0])}}
+            extra = ["cfg3_gauss9d",            # configs[2] whole, the paper's rule
+                     "cfg2_sin6d_depth2",       # configs[1] under the paper's rule (no budget), levels 1-2 of 3 (~2.4 s)
+                     "cfg5_sin6d_depth4_B1"]    # configs[4] to depth 4 with one refined cell per level (~8 s)
+            for name in extra:
+                if name == args.workload:
+                    continue
+                wx = wl[name]
+                itx = B.from_workload(wx, math=math, max_cells_per_level=capacity_for(wx))
+                n_warm = 2 if wx.name == "cfg3_gauss9d" else 0       # the long ones are their own warm-up: same kernel as the timed steps above
+                for _ in range(n_warm + 1):
+                    itx.run(stream.cuda_stream)
+                vx, sx = itx.result()
+                stx = itx.stats()
+                line["time_to_result"][name] = {
+                    "ms": stx.total_ms, "value": float(vx[0]), "std": float(sx[0]), "evals": int(stx.total_evals),
+                    "evals_per_s": stx.total_evals / (stx.total_ms * 1e-3),
+                    "cells_per_level": [int(stx.level[l].n_cells) for l in range(stx.levels)],
+                    "flagged_per_level": [int(stx.level[l].n_flagged) for l in range(stx.levels)],
+                    "refined_per_level": [int(stx.level[l].n_refined) for l in range(stx.levels)],
+                    "deviation": DEVIATIONS.get(name)}
+                itx.close()
             # BASELINE.json configs[0] is launch-bound (microseconds of arithmetic): kernel by kernel vs one CUDA graph
             w1 = wl["cfg1_sin3d_f64"]
             for key, graph in (("cfg1_sin3d_f64", False), ("cfg1_sin3d_f64_graph", True)):

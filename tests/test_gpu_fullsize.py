@@ -27,6 +27,7 @@ from tests import helpers as H
 pytestmark = pytest.mark.gpu
 
 N_SAMPLED_UNITS = {"cfg2_sin6d_depth3_B16": 24, "cfg2_sin6d_depth2": 16, "cfg3_gauss9d": 40, "cfg4_batched4d_B4": 200, "cfg5_sin6d_level1": 12,
+                   "cfg5_sin6d_depth4_B1": 10, "cfg5_sin6d_depth4_B1+spread": 6,
                    "cfg12_gauss12d": 24}
 
 
@@ -45,15 +46,18 @@ def _closed(w, inst=0):
 
 
 def _bench_integrator(name, w):
+    """'+spread' after a workload name = bench.py --budget-order spread (R14: the budget keeps the largest spreads)."""
     cap = bench.capacity_for(w)
-    it = B.from_workload(w, math=B.MATH_EXACT, keep_level_stats=True, max_cells_per_level=cap)
+    order = B.BUDGET_LARGEST_SPREAD if name.endswith("+spread") else B.BUDGET_PATH_ORDER
+    it = B.from_workload(w, math=B.MATH_EXACT, keep_level_stats=True, max_cells_per_level=cap, budget_order=order)
     it.use_torch_workspace()
     return it
 
 
 @pytest.mark.parametrize("name", sorted(N_SAMPLED_UNITS))
 def test_fullsize_sampled_units_and_full_control(name):
-    w = bench.workloads()[name]
+    w = bench.workloads()[name.split("+")[0]]
+    by_spread = name.endswith("+spread")
     cfg = H.oracle_config(w)
     rng = np.random.default_rng(2024)
     it = _bench_integrator(name, w)
@@ -114,7 +118,7 @@ def test_fullsize_sampled_units_and_full_control(name):
         assert np.abs(gl.mu - mu).max() <= 1e-11 * sc
         assert np.abs(gl.s - s).max() <= 1e-9 * sc
         tau_c, refined, lv, lvar = H.host_control(gl.mu, gl.s, k, level, w.depth, w.sigma_multiplier, inst,
-                                                  budget=w.max_groups_per_level)
+                                                  budget=w.max_groups_per_level, largest_spread=by_spread)
         assert np.abs(gl.tau - tau_c).max() <= 1e-11 * max(tau_c.max(), 1e-300)
         diff = np.nonzero(gl.refined.astype(bool) != refined)[0]
         if len(diff):    # only exact ties between s and a re-derived tau may differ (and then the budget shifts)
@@ -124,6 +128,13 @@ def test_fullsize_sampled_units_and_full_control(name):
             lv = np.bincount(inst[acc], weights=gl.mu[acc], minlength=w.n_instances)
             lvar = np.bincount(inst[acc], weights=gl.s[acc] ** 2, minlength=w.n_instances)
         assert st.level[level - 1].n_refined == int(refined.sum())
+        n_flag = int(((gl.s > gl.tau) & (level < w.depth)).sum())      # zmc_stats counts every flagged cell, kept by the budget or not
+        assert st.level[level - 1].n_flagged == n_flag, (level, st.level[level - 1].n_flagged, n_flag)
+        if name.startswith("cfg5_sin6d_depth4_B1"):     # compaction of ~4e4 flagged cells in one 262144-cell group, then 72-bit paths
+            assert n == 262144 and (level == w.depth or 2e4 < n_flag < 8e4), (level, n_flag)
+        if name == "cfg5_sin6d_depth4_B1+spread" and level == 4:
+            # the first flagged cell in path order has a small index; the largest spread sits anywhere, so these paths pass 64 bits
+            assert max(paths).bit_length() > 64, max(paths).bit_length()
         val[: len(lv)] += lv
         var[: len(lvar)] += lvar
         idx = np.nonzero(refined)[0]
