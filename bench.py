@@ -181,8 +181,7 @@ def oracle_sample(w, n_units, seed_offset=0):
     Returns (evals, seconds)."""
     import numpy as np
     import oracle as O
-    from tests import helpers as H
-    cfg = H.oracle_config(w)
+    cfg = O.config_from_workload(w)
     rng = np.random.default_rng(1234 + seed_offset)
     cells = rng.integers(0, w.k, size=n_units)
     t0 = time.perf_counter()

@@ -35,7 +35,7 @@ extern "C" {
 typedef enum zmc_status {
     ZMC_OK = 0,
     ZMC_ERR_ARG = -1,          /* null pointer, non-finite or empty bounds, counts < 1 ... */
-    ZMC_ERR_RANGE = -2,        /* path > 80 bits, g^depth > 2^32, N*D/4 >= 2^32 - 4096, trials > 255, depth > 15, dim > 16 */
+    ZMC_ERR_RANGE = -2,        /* path > 80 bits, g^depth > 2^32, N*D >= 2^34 - 2^14, trials > 255, depth > 15, dim > 16 (R3) */
     ZMC_ERR_NO_INTEGRAND = -3, /* zmc_run before zmc_set_integrand* */
     ZMC_ERR_COMPILE = -4,      /* NVRTC failed; the log is in zmc_last_error */
     ZMC_ERR_CUDA = -5,         /* a CUDA runtime call failed (or no device) */
@@ -90,7 +90,9 @@ typedef struct zmc_ctx zmc_ctx; /* opaque; owned by the library between zmc_crea
  *   trials             n1 = T independent repetitions per cell, 1..255
  *   depth              L = number of levels evaluated; depth 1 = no refinement, 1..15
  *   sigma_multiplier   m in the threshold tau = mean(s) + m * pstd(s) of one sibling group (R6)
- *   seed               Philox seed (R3) */
+ *   seed               Philox seed (R3)
+ * Limits (else ZMC_ERR_RANGE): samples_per_cell * dim < 2^34 - 2^14, depth * dim * log2(g) <= 80, g^depth <= 2^32, g^dim <= 2^40.
+ * On failure *out is NULL -- there is nothing to destroy -- and zmc_last_error(NULL) gives the reason. */
 int zmc_create(zmc_ctx** out, int dim, const double* lower, const double* upper, int divisions_per_axis,
                uint64_t samples_per_cell, int trials, int depth, double sigma_multiplier, uint64_t seed);
 
@@ -100,16 +102,22 @@ int zmc_create(zmc_ctx** out, int dim, const double* lower, const double* upper,
 int zmc_set_integrand(zmc_ctx* ctx, int builtin_id, const double* params, int params_per_instance, int n_instances);
 
 /* Choose a user integrand given as CUDA source, JIT-compiled with NVRTC for sm_100a together with the
- * sampling kernel so that it inlines. cuda_src [host] must define, for the precision in force when
- * zmc_run is called,
+ * sampling kernel so that it inlines. cuda_src [host] must define
  *     __device__ float  fn_name(const float*  x, int dim, const float*  p, int np)   (ZMC_F32)
  *     __device__ double fn_name(const double* x, int dim, const double* p, int np)   (ZMC_F64)
  * x = the sample point, p = this instance's parameters. Parity with a CPU holds for built-ins only.
+ * The program is compiled DURING THIS CALL, for the precision, math mode and spread in force now (the default precision is
+ * ZMC_F64), so that a compile error surfaces here with the NVRTC log in zmc_last_error: a source that defines one overload
+ * only needs that precision set BEFORE this call. A later zmc_set_option(ZMC_OPT_PRECISION / MATH / SPREAD) recompiles at
+ * once; if that fails it returns ZMC_ERR_COMPILE and the context keeps its previous, working setting.
  * Compiled programs are cached per process, and on disk as well if the environment variable ZMC_CACHE_DIR names a
  * writable directory (keyed by the complete program text; a stale or foreign file is ignored). */
 int zmc_set_integrand_source(zmc_ctx* ctx, const char* cuda_src, const char* fn_name, const double* params,
                              int params_per_instance, int n_instances);
 
+/* Returns ZMC_ERR_ARG for an unknown key or a value out of range, ZMC_ERR_STATE for a value that changes the workspace
+ * layout (KEEP_LEVEL_STATS, MAX_CELLS_PER_LEVEL, TARGET_ITEMS, SPREAD, BUDGET_ORDER) after zmc_set_workspace has fixed a
+ * caller-owned workspace and a run has laid it out. On any error the context is unchanged. */
 int zmc_set_option(zmc_ctx* ctx, int key, int64_t value);
 
 /* Device memory the run needs under the options in force. Optional: without zmc_set_workspace the
@@ -168,6 +176,16 @@ int zmc_level_cells(zmc_ctx* ctx, int level, uint64_t capacity, uint64_t* n_cell
                     uint64_t* path_lo, uint32_t* path_hi, double* mu, double* s, double* tau, uint8_t* refined,
                     double* S);
 
+/* The same arrays for the cells [first_cell, first_cell + count) of the level only (a level of a deep, unbudgeted tree can
+ * hold 10^8 cells and more: BASELINE.json configs[1] at depth 3). Every non-NULL [host] array holds count entries (S: count*T).
+ * ZMC_ERR_ARG if the range passes the level's cell count.
+ * Both dump calls take mu, s, tau, refined, S and the parents' (instance, path) from device memory as the kernels wrote them;
+ * a cell's own path P' = P*k + j is then formed on the host from its parent's path P and its position j in the group (128-bit
+ * integer arithmetic). The device forms the same P' per work item for the Philox counter and does not store it. */
+int zmc_level_cells_range(zmc_ctx* ctx, int level, uint64_t first_cell, uint64_t count, uint32_t* instance,
+                          uint64_t* path_lo, uint32_t* path_hi, double* mu, double* s, double* tau, uint8_t* refined,
+                          double* S);
+
 /* Per-(cell, trial) sums of f^2 of one level, Q[c*T + t], FP64 (R13); needs ZMC_OPT_KEEP_LEVEL_STATS and
  * ZMC_SPREAD_SAMPLES. Q [host] capacity*T doubles, capacity >= the level's cell count. */
 int zmc_level_sumsq(zmc_ctx* ctx, int level, uint64_t capacity, double* Q);
@@ -184,17 +202,9 @@ int zmc_debug_words(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t 
 int zmc_debug_points(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
                      const uint32_t* coords, int trial, uint64_t n, double* x, double* f);
 
-/* Issue-rate microbenchmarks of the pipes the path uses (roofline denominator).
- * which: 0 IMAD.WIDE.U32, 1 LOP3, 2 IMAD.WIDE+LOP3 (Philox round mix), 3 FFMA, 4 FADD, 5 DADD, 6 F2F.F64.F32 + F2F.F32.F64 (pair),
- *        7 MUFU.SIN, 8 MUFU.EX2, 9 DFMA, 10 Philox4x32-10 calls, 11 I2F.F64.U32 + F2I.U32.F64 (pair), 12 LEA.HI,
- *        13 IMAD (lo), 14 IMAD.HI.U32, 15 64-bit add (IADD3 + IADD3.X, counted as one), 16 IMAD.WIDE.U32 by a register
- *        100 + 10*X + j: Philox4x32-10 calls, each followed by K = {0, 10, 20, 40}[j] extra independent instructions of
- *        kind X = 1 LOP3, 2 FFMA, 3 FADD, 4 DADD, 5 FFMA2, 6 IMAD, 7 SHF (the cost of an instruction next to the generator)
- * Returns warp-instructions (which 10 and >= 100: Philox calls x 32 lanes) per SM per clock in *per_sm_clk and the
- * SM clock seen (clock64 ticks / event time) in *sm_mhz. */
-int zmc_microbench(int which, void* cuda_stream, double* per_sm_clk, double* sm_mhz);
-
-const char* zmc_last_error(const zmc_ctx* ctx);   /* "" if none; valid until the next call on ctx */
+/* The reason of the last failure on ctx ("" if none; valid until the next call on ctx). ctx == NULL: the reason of the calling
+ * thread's last failed zmc_create (valid until that thread's next zmc_create). */
+const char* zmc_last_error(const zmc_ctx* ctx);
 const char* zmc_status_string(int status);
 void zmc_destroy(zmc_ctx* ctx);
 

@@ -80,6 +80,20 @@ def lib():
     return L
 
 
+def config_from_workload(w, **over) -> "Config":
+    """A seeded workload description (any object with the fields of paper_1902_07916_b200.workloads.Workload: plain sizes,
+    names and parameter arrays -- this package imports nothing from the product) as an oracle Config."""
+    integrand = {"const": CONST, "linear": LINEAR, "sin_sum": SIN_SUM, "exp_quad": EXP_QUAD}[w.integrand]
+    precision = {"f64": F64, "f32": F32}[w.precision]
+    cfg = Config(dim=w.dim, lower=list(w.lower), upper=list(w.upper), g=w.g, n_samples=w.n_samples,
+                 trials=w.trials, depth=w.depth, sigma_multiplier=w.sigma_multiplier, seed=w.seed,
+                 integrand=integrand, precision=precision, params=w.params, n_instances=w.n_instances,
+                 max_groups_per_level=w.max_groups_per_level)
+    for k, v in over.items():
+        setattr(cfg, k, v)
+    return cfg
+
+
 def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 

@@ -266,7 +266,8 @@ const char* check_config(const orc_config* c) {
     if (c->trials < 1 || c->trials > 255) return "trials out of range (1..255)";
     if (c->depth < 1 || c->depth > 15) return "depth out of range (1..15)";
     if (c->n_samples < 1) return "n_samples < 1";
-    if ((u128)c->n_samples * (u128)c->dim > ((u128)1 << 34)) return "N*D/4 >= 2^32";
+    /* R3: call indices are 32-bit; the limit is stated once for both implementations (R3): N*D < 2^34 - 2^14 */
+    if ((u128)c->n_samples * (u128)c->dim >= ((u128)1 << 34) - ((u128)1 << 14)) return "N*D >= 2^34 - 2^14";
     if (c->n_instances < 1) return "n_instances < 1";
     if (!(c->sigma_multiplier == c->sigma_multiplier)) return "sigma_multiplier is NaN";
     for (int d = 0; d < c->dim; ++d)

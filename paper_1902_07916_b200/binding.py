@@ -31,8 +31,8 @@ MATH_EXACT, MATH_FAST = 0, 1
 MAX_DEPTH = 15
 
 EXPORTS = ["zmc_create", "zmc_set_integrand", "zmc_set_integrand_source", "zmc_set_option", "zmc_workspace_bytes",
-           "zmc_set_workspace", "zmc_run", "zmc_result", "zmc_stats", "zmc_level_cells", "zmc_level_sumsq", "zmc_debug_words",
-           "zmc_debug_points", "zmc_microbench", "zmc_last_error", "zmc_status_string", "zmc_destroy"]
+           "zmc_set_workspace", "zmc_run", "zmc_result", "zmc_stats", "zmc_level_cells", "zmc_level_cells_range", "zmc_level_sumsq", "zmc_debug_words",
+           "zmc_debug_points", "zmc_last_error", "zmc_status_string", "zmc_destroy"]
 
 _INTEGRAND_ID = {W.CONST: CONST, W.LINEAR: LINEAR, W.SIN_SUM: SIN_SUM, W.EXP_QUAD: EXP_QUAD}
 _PRECISION_ID = {W.F64: F64, W.F32: F32}
@@ -64,13 +64,16 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    path = LIB_PATH
-    try:
-        from . import build as _build
-        path = _build.build()
-    except Exception:
-        if not os.path.exists(LIB_PATH):
-            raise
+    from . import build as _build
+    if os.path.exists(_build.NVCC):
+        path = _build.build()        # rebuilds iff the sources changed; a compile or link error is raised, never papered over
+    elif os.path.exists(LIB_PATH):
+        path = LIB_PATH              # no compiler on this machine: the shipped library as it is
+        if not _build.is_current() and os.environ.get("ZMC_ALLOW_STALE") != "1":
+            raise RuntimeError("libzmc.so does not match the sources (stamp mismatch) and there is no nvcc to rebuild it; "
+                               "set ZMC_ALLOW_STALE=1 to load it anyway")
+    else:
+        raise RuntimeError("libzmc.so is missing and nvcc (%s) is not available to build it" % _build.NVCC)
     L = C.CDLL(path)
     vp, dp, u32p, u64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
     L.zmc_create.argtypes = [C.POINTER(vp), C.c_int, dp, dp, C.c_int, C.c_uint64, C.c_int, C.c_int, C.c_double, C.c_uint64]
@@ -83,10 +86,10 @@ def lib():
     L.zmc_result.argtypes = [vp, dp, dp]
     L.zmc_stats.argtypes = [vp, C.POINTER(Stats)]
     L.zmc_level_cells.argtypes = [vp, C.c_int, C.c_uint64, u64p, u32p, u64p, u32p, dp, dp, dp, C.POINTER(C.c_uint8), dp]
+    L.zmc_level_cells_range.argtypes = [vp, C.c_int, C.c_uint64, C.c_uint64, u32p, u64p, u32p, dp, dp, dp, C.POINTER(C.c_uint8), dp]
     L.zmc_level_sumsq.argtypes = [vp, C.c_int, C.c_uint64, dp]
     L.zmc_debug_words.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_uint64, C.c_uint64, u32p]
     L.zmc_debug_points.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, C.c_uint64, dp, dp]
-    L.zmc_microbench.argtypes = [C.c_int, vp, dp, dp]
     L.zmc_last_error.argtypes = [vp]
     L.zmc_last_error.restype = C.c_char_p
     L.zmc_status_string.argtypes = [C.c_int]
@@ -129,12 +132,8 @@ class Integrator:
         up = np.ascontiguousarray(upper, dtype=np.float64)
         rc = self._L.zmc_create(C.byref(self._h), dim, _dp(lo), _dp(up), divisions_per_axis, samples_per_cell,
                                 trials, depth, float(sigma_multiplier), seed)
-        if rc != OK:
-            msg = self._L.zmc_last_error(self._h).decode() if self._h else self._L.zmc_status_string(rc).decode()
-            if self._h:
-                self._L.zmc_destroy(self._h)
-                self._h = C.c_void_p()
-            raise ZmcError(rc, msg)
+        if rc != OK:      # no context exists after a failed zmc_create; the reason is zmc_last_error(NULL)
+            raise ZmcError(rc, self._L.zmc_last_error(None).decode() or self._L.zmc_status_string(rc).decode())
         self._ws = None
 
     def _check(self, rc):
@@ -230,6 +229,18 @@ class Integrator:
         path = [(int(h) << 64) | int(l) for h, l in zip(phi, plo)]
         return LevelCells(inst, path, mu, s, tau, ref, S)
 
+    def level_cells_range(self, level: int, first: int, count: int) -> LevelCells:
+        inst = np.zeros(count, dtype=np.uint32)
+        plo = np.zeros(count, dtype=np.uint64)
+        phi = np.zeros(count, dtype=np.uint32)
+        mu, s, tau = np.zeros(count), np.zeros(count), np.zeros(count)
+        ref = np.zeros(count, dtype=np.uint8)
+        S = np.zeros((count, self.trials))
+        self._check(self._L.zmc_level_cells_range(self._h, level, first, count, _ptr(inst, C.c_uint32), _ptr(plo, C.c_uint64),
+                                                  _ptr(phi, C.c_uint32), _dp(mu), _dp(s), _dp(tau), _ptr(ref, C.c_uint8), _dp(S)))
+        path = [(int(h) << 64) | int(l) for h, l in zip(phi, plo)]
+        return LevelCells(inst, path, mu, s, tau, ref, S)
+
     def level_sumsq(self, level: int, n_cells: int) -> np.ndarray:
         Q = np.zeros((n_cells, self.trials))
         self._check(self._L.zmc_level_sumsq(self._h, level, n_cells, _dp(Q)))
@@ -271,11 +282,3 @@ def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool 
     if max_cells_per_level or w.max_cells_per_level:
         it.set_option(OPT_MAX_CELLS_PER_LEVEL, max_cells_per_level or w.max_cells_per_level)
     return it
-
-
-def microbench(which: int, stream: int = 0):
-    r, mhz = C.c_double(), C.c_double()
-    rc = lib().zmc_microbench(which, C.c_void_p(stream), C.byref(r), C.byref(mhz))
-    if rc != OK:
-        raise ZmcError(rc, lib().zmc_status_string(rc).decode())
-    return r.value, mhz.value

@@ -5,9 +5,11 @@
 Steps
   1. csrc/zmc_device.cuh -> csrc/zmc_device_src.inc (the same text as a C++ raw string literal,
      handed to NVRTC at run time for user integrands and for 12 < D <= 16);
-  2. nvcc -c, in parallel: zmc_lib.cu, zmc_microbench.cu and zmc_inst.cu once per pre-compiled
+  2. nvcc -c, in parallel: zmc_lib.cu and zmc_inst.cu once per pre-compiled
      (precision, math mode, integrand) combination;
   3. nvcc -shared -cudart static -> paper_1902_07916_b200/libzmc.so.
+build_microbench() makes the pipe-rate probes of csrc/zmc_microbench.cu a library of their own
+(libzmc_microbench.so, used by `python -m paper_1902_07916_b200.microbench` only): they are not part of the product ABI.
 
 Flags: -gencode arch=compute_100a,code=sm_100a (B200 only), -lineinfo (ncu source pages),
 --fmad=false (every fused multiply-add in the device code is written explicitly; R8).
@@ -59,8 +61,7 @@ def _write_source_inc() -> str:
 
 
 def _sources():
-    jobs = [("zmc_lib", os.path.join(CSRC, "zmc_lib.cu"), []),
-            ("zmc_microbench", os.path.join(CSRC, "zmc_microbench.cu"), [])]
+    jobs = [("zmc_lib", os.path.join(CSRC, "zmc_lib.cu"), [])]
     for p, m, i in COMBOS:
         jobs.append(("zmc_inst_%d_%d_%d" % (p, m, i), os.path.join(CSRC, "zmc_inst.cu"),
                      ["-DZMC_INST_PREC=%d" % p, "-DZMC_INST_MODE=%d" % m, "-DZMC_INST_ID=%d" % i]))
@@ -70,13 +71,19 @@ def _sources():
 def _stamp() -> str:
     h = hashlib.sha256()
     for name in sorted(os.listdir(CSRC)):
-        if name.endswith((".cu", ".cuh", ".h")):
+        if name.endswith((".cu", ".cuh", ".h")) and name != "zmc_microbench.cu":
             h.update(name.encode())
             h.update(open(os.path.join(CSRC, name), "rb").read())
     h.update(open(os.path.join(os.path.dirname(HERE), "include", "zmc.h"), "rb").read())
     h.update(open(os.path.abspath(__file__), "rb").read())
     h.update(" ".join(NVCC_FLAGS).encode())
     return h.hexdigest()
+
+
+def is_current() -> bool:
+    """True if libzmc.so was built from exactly these sources and flags."""
+    stamp_file = os.path.join(OBJ, "stamp.txt")
+    return os.path.exists(LIB) and os.path.exists(stamp_file) and open(stamp_file).read() == _stamp()
 
 
 def _compile(job, verbose):
@@ -113,6 +120,22 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with open(stamp_file, "w") as f:
         f.write(stamp)
     return LIB
+
+
+MICROBENCH_LIB = os.path.join(HERE, "libzmc_microbench.so")
+
+
+def build_microbench(force: bool = False) -> str:
+    """The issue-rate probes (profiles/r1_microbench.md) as their own small library; not linked into libzmc.so."""
+    src = os.path.join(CSRC, "zmc_microbench.cu")
+    deps = [src, os.path.join(CSRC, "zmc_device.cuh")]
+    if not force and os.path.exists(MICROBENCH_LIB) and all(os.path.getmtime(MICROBENCH_LIB) >= os.path.getmtime(d) for d in deps):
+        return MICROBENCH_LIB
+    cmd = [NVCC, *NVCC_FLAGS, "-shared", "-cudart", "static", "-o", MICROBENCH_LIB, src]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed for zmc_microbench:\n%s\n%s" % (" ".join(cmd), r.stderr[-6000:]))
+    return MICROBENCH_LIB
 
 
 if __name__ == "__main__":

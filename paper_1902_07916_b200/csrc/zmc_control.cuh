@@ -39,6 +39,7 @@ struct ZmcCtlArgs {
     zu64 k, N;
     zu32 sample_groups;     /* sample groups per unit = ceil(N / SG) */
     zu32 target_items, min_chunk_groups;
+    zu32 trial_loop;        /* 1: the sampling kernel in use honours ZmcLevelInfo::trials_per_item (ZmcTune::TRIAL_LOOP) */
     double V;               /* cell volume at this level (R2) */
     double m;               /* sigma multiplier */
     zu64 budget;            /* R12; ~0 = off */
@@ -70,7 +71,7 @@ struct ZmcCtlArgs {
     double* Q;              /* [cell*T + t], or nullptr */
     /* R14: the budget keeps the largest spreads */
     zu32 budget_order;      /* 0: first B flagged cells in path order (R12) ; 1: the B largest spreads */
-    zu64* piv;              /* [instance] key (bits of s) of the B-th largest flagged spread; 0 = keep every flagged cell */
+    zu64* piv;              /* [instance] key (bits of s) of the B-th largest flagged spread; 0 with quota ~0 = keep every flagged cell */
     zu64* quota;            /* [instance] how many cells with s == pivot are kept (the first in path order) */
     zu64* cnt_gt;           /* [group] flagged cells with key > pivot */
     zu64* cnt_eq;           /* [group] flagged cells with key == pivot */
@@ -93,7 +94,11 @@ __device__ __forceinline__ void zmc_plan_level(ZmcLevelInfo& li, zu64 n_groups, 
     const zu32 cg = (zu32)(((zu64)c.sample_groups + nch - 1) / nch);
     li.chunk_groups = cg;
     li.n_chunks = (zu32)(((zu64)c.sample_groups + cg - 1) / cg);    /* 64-bit: sample_groups may be within cg of 2^32 */
-    li.n_items = units * li.n_chunks;
+    /* a level with at least target_items CELLS has work items to spare: one item = all T trials of a cell, so that item decoding and
+     * cell geometry are paid once per cell (visible at small N: BASELINE.json configs[3] has 4096 samples per unit) */
+    li.trials_per_item = (c.trial_loop && li.n_chunks == 1u && li.n_cells >= c.target_items) ? c.T : 1u;
+    li.reserved = 0u;
+    li.n_items = (units / li.trials_per_item) * li.n_chunks;
     li.work_ctr = 0;
     li.n_flagged = 0;
     li.n_refined = 0;
@@ -126,7 +131,7 @@ __global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) {
         for (zu32 l = 0; l <= c.L + 1; ++l) {
             ZmcLevelInfo z;
             z.n_groups = z.n_cells = z.n_items = z.work_ctr = z.n_flagged = z.n_refined = 0;
-            z.n_chunks = 1; z.chunk_groups = c.sample_groups;
+            z.n_chunks = 1; z.chunk_groups = c.sample_groups; z.trials_per_item = 1; z.reserved = 0;
             if (l != 1) c.info[l] = z;
         }
         ZmcLevelInfo li;
@@ -335,7 +340,7 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid
 /* ------------------------------------------------------------------ R14: the budget keeps the largest spreads */
 /* One block per instance: if more than B cells are flagged, radix-select (8 passes of 8 bits over the bit pattern
  * of s, which orders positive doubles) the B-th largest flagged spread -> piv, and how many cells equal to it are
- * kept -> quota = B - #(s > pivot). Otherwise piv = 0: every flagged cell has s > tau >= 0, i.e. key > 0. */
+ * kept -> quota = B - #(s > pivot). Otherwise piv = 0 and quota = all: no flagged cell is dropped (s >= +0, i.e. key >= 0). */
 __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu32 hist[256];
     __shared__ zu64 sh_prefix, sh_need, sh_above;
@@ -343,8 +348,8 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __gr
         const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
         const zu64 cb = (g1 > g0) ? c.excl[g1 - 1] + c.cnt[g1 - 1] - c.excl[g0] : 0ull;
         __syncthreads();
-        if (cb <= c.budget) {
-            if (threadIdx.x == 0) { c.piv[b] = 0ull; c.quota[b] = 0ull; }
+        if (cb <= c.budget) {   /* nothing to cut: every flagged cell is kept -- also those with s == +0 (key 0), flagged when tau < 0 (m < 0) */
+            if (threadIdx.x == 0) { c.piv[b] = 0ull; c.quota[b] = ~0ull; }
             continue;
         }
         if (threadIdx.x == 0) { sh_prefix = 0ull; sh_need = c.budget; sh_above = 0ull; }

@@ -28,6 +28,7 @@ typedef unsigned long long zu64;
 typedef int zi32;
 
 #define ZMC_DEV_MAX_DIM 16
+#define ZMC_HAS_TPI 1
 #ifndef ZMC_BLOCK_THREADS
 #define ZMC_BLOCK_THREADS 128
 #endif
@@ -48,12 +49,15 @@ typedef int zi32;
 struct ZmcLevelInfo {
     zu64 n_groups;      /* parents = sibling groups at this level */
     zu64 n_cells;       /* n_groups * k */
-    zu64 n_items;       /* n_cells * T * n_chunks work items */
+    zu64 n_items;       /* n_cells * (T / trials_per_item) * n_chunks work items */
     zu64 work_ctr;      /* the persistent grid's item counter */
     zu64 n_flagged;     /* cells with s > tau */
     zu64 n_refined;     /* flagged cells passed on (after budget and capacity) */
     zu32 n_chunks;      /* sample chunks per (cell, trial) unit */
     zu32 chunk_groups;  /* sample groups per chunk */
+    zu32 trials_per_item; /* 1, or T on levels with many cells: one warp takes all trials of a cell, so that the item decoding
+                             and the cell geometry are paid once per cell instead of once per trial (n_chunks == 1 then) */
+    zu32 reserved;
 };
 
 struct ZmcSampleArgs {
@@ -174,8 +178,11 @@ __device__ __forceinline__ float zmc_zsin(float a) {
  * polynomial p ~ exp(r); exp(e) = p * 2^n is assembled as an FP64 number by adding n to the
  * exponent field of (double)p, so the FP64 exponent range is available (R9: the 9-D Gaussian's
  * samples at level 1 lie far below FP32's range). |e| > 708 and NaN take the slow branch. */
+/* CHK = false: the caller has proved |e| <= 708 for every sample of the work item (ZmcIntegrand::setup, "range proof"),
+ * so the test, its branch and the special values are not in the loop at all; the arithmetic is the same. */
+template <bool CHK = true>
 __device__ __forceinline__ double zmc_zexp_value(float e) {
-    if (!(fabsf(e) <= 708.0f)) {
+    if (CHK && !(fabsf(e) <= 708.0f)) {
         if (e < 0.0f) return 0.0;
         if (e > 0.0f) return __longlong_as_double(0x7FF0000000000000ll);
         return __longlong_as_double(0x7FF8000000000000ll);
@@ -203,8 +210,9 @@ __device__ __forceinline__ double zmc_zexp_value(float e) {
 }
 
 /* fast mode: the same split e*log2e = n + r, with 2^r from MUFU.EX2 */
+template <bool CHK = true>
 __device__ __forceinline__ double zmc_fexp_value(float e) {
-    if (!(fabsf(e) <= 708.0f)) {
+    if (CHK && !(fabsf(e) <= 708.0f)) {
         if (e < 0.0f) return 0.0;
         if (e > 0.0f) return __longlong_as_double(0x7FF0000000000000ll);
         return __longlong_as_double(0x7FF8000000000000ll);
@@ -261,13 +269,15 @@ __device__ __forceinline__ zf2 zmc_zsin2(zf2 a) {
 }
 
 /* zmc_zexp_value on a pair: packed reduction and polynomial, then each component assembled as there */
+template <bool CHK>
 __device__ __forceinline__ double zmc_zexp_finish(float e, float t, float p) {
     const double dp = (double)p;
     double v = __hiloint2double(__double2hiint(dp) + (zi32)(__float_as_uint(t) << 20), __double2loint(dp));
-    if (!(fabsf(e) <= 708.0f))
+    if (CHK && !(fabsf(e) <= 708.0f))
         v = (e < 0.0f) ? 0.0 : ((e > 0.0f) ? __longlong_as_double(0x7FF0000000000000ll) : __longlong_as_double(0x7FF8000000000000ll));
     return v;
 }
+template <bool CHK>
 __device__ __forceinline__ void zmc_zexp2(zf2 e, double& fa, double& fb) {
     const float LOG2E = __uint_as_float(0x3fb8aa3bu);
     const float MAGIC = __uint_as_float(0x4b400000u);
@@ -285,8 +295,8 @@ __device__ __forceinline__ void zmc_zexp2(zf2 e, double& fa, double& fb) {
     p = zmc_fma2(p, r, zmc_bc(E2));
     p = zmc_fma2(p, r, zmc_bc(1.0f));
     p = zmc_fma2(p, r, zmc_bc(1.0f));
-    fa = zmc_zexp_finish(zmc_lo(e), zmc_lo(t), zmc_lo(p));
-    fb = zmc_zexp_finish(zmc_hi(e), zmc_hi(t), zmc_hi(p));
+    fa = zmc_zexp_finish<CHK>(zmc_lo(e), zmc_lo(t), zmc_lo(p));
+    fb = zmc_zexp_finish<CHK>(zmc_hi(e), zmc_hi(t), zmc_hi(p));
 }
 
 /* ------------------------------------------------------------------ R2 + R4: cell geometry and the word -> point map */
@@ -332,6 +342,12 @@ struct ZmcMapF64 {
 #define ZMC_PACKED_EXP_POLY(D) ((D) <= 8)
 #endif
 
+/* two copies of the sample loop (with and without zexp's range test) pay where the polynomial is packed; with the scalar
+ * polynomial of D >= 9 ptxas needs 50-60 more registers for them (measured) and most cells of a narrow Gaussian are out of range anyway */
+#ifndef ZMC_RANGE_PROOF
+#define ZMC_RANGE_PROOF(D) ZMC_PACKED_EXP_POLY(D)
+#endif
+
 /* ------------------------------------------------------------------ integrands */
 /* Each integrand policy has
  *   setup(args, instance, coords)  once per work item: geometry and this instance's parameters
@@ -354,6 +370,10 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
     float lin[ID == ZMC_ID_LINEAR ? D_ : 1];
     const float* up;    /* user parameters */
     zi32 unp;
+    /* EXP_QUAD: true if |e| = |a|*q <= 708 is proved for every point of this cell, so that the sample loop can run
+     * without the per-sample range test of zexp (same arithmetic, fewer instructions); false = test every sample */
+    static constexpr bool HAS_RANGE_PROOF = (ID == ZMC_ID_EXP_QUAD) && ZMC_RANGE_PROOF(D_);
+    bool in_range;
 
     __device__ __forceinline__ void setup(const ZmcSampleArgs& a, zu32 inst, const zu32* coords) {
         const double* p = a.params + (zu64)inst * (zu64)a.ppi;
@@ -371,8 +391,23 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
         }
         up = a.params_f32 + (zu64)inst * (zu64)a.ppi;
         unp = a.ppi;
+        in_range = false;
+        if (HAS_RANGE_PROOF) {
+            /* x_d = fmaf(u', wf, base) is monotone in u' in [1, 2): |x_d| <= max(|fl(wf+base)|, |fl(2wf+base)|) =: m_d.
+             * q <= (sum m_d^2)(1 + D*2^-23) in FP32 ; the bound carries a 2^-7 margin and the limit 700 leaves 8 more */
+            float qmax = 0.0f;
+#pragma unroll
+            for (int d = 0; d < D_; ++d) {
+                const float xa = fabsf(__fmaf_rn(1.0f, map.wf[d], map.base[d]));
+                const float xb = fabsf(__fmaf_rn(2.0f, map.wf[d], map.base[d]));
+                const float md = fmaxf(xa, xb);
+                qmax = __fmaf_rn(md, md, qmax);
+            }
+            in_range = __fmul_rn(__fmul_rn(fabsf(c0), qmax), 1.0078125f) <= 700.0f;      /* NaN: false */
+        }
     }
 
+    template <bool CHK = true>
     __device__ __forceinline__ double eval(const zu32* w, double* xout) const {
         float x[D_];
 #pragma unroll
@@ -400,8 +435,8 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
 #pragma unroll
             for (int d = 1; d < D_; ++d) q = __fmaf_rn(x[d], x[d], q);
             const float e = __fmul_rn(c0, q);
-            if (MODE == ZMC_MODE_FAST) return zmc_fexp_value(e);
-            return zmc_zexp_value(e);
+            if (MODE == ZMC_MODE_FAST) return zmc_fexp_value<CHK>(e);
+            return zmc_zexp_value<CHK>(e);
         }
 #ifdef ZMC_USER_FN
         if (ID == ZMC_ID_USER) return (double)ZMC_USER_FN((const float*)x, D_, up, unp);
@@ -412,8 +447,9 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
     /* Two samples at once on the packed FP32 instructions: component-wise the operation sequence of eval(),
      * hence the same bits (checked by the P1 parity test through zmc_points_kernel). */
     static constexpr bool HAS_PACKED = (ID == ZMC_ID_SIN_SUM || ID == ZMC_ID_EXP_QUAD || ID == ZMC_ID_LINEAR);
+    template <bool CHK = true>
     __device__ __forceinline__ void eval2(const zu32* wa, const zu32* wb, double& fa, double& fb) const {
-        if (!HAS_PACKED) { fa = eval(wa, nullptr); fb = eval(wb, nullptr); return; }
+        if (!HAS_PACKED) { fa = eval<CHK>(wa, nullptr); fb = eval<CHK>(wb, nullptr); return; }
         zf2 x[D_];
 #pragma unroll
         for (int d = 0; d < D_; ++d) x[d] = map.x2(d, wa[d], wb[d]);
@@ -446,13 +482,13 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
             for (int d = 1; d < D_; ++d) q = zmc_fma2(x[d], x[d], q);
             const zf2 e = zmc_mul2(zmc_bc(c0), q);
             if (MODE == ZMC_MODE_FAST) {
-                fa = zmc_fexp_value(zmc_lo(e));
-                fb = zmc_fexp_value(zmc_hi(e));
+                fa = zmc_fexp_value<CHK>(zmc_lo(e));
+                fb = zmc_fexp_value<CHK>(zmc_hi(e));
             } else if (ZMC_PACKED_EXP_POLY(D_)) {
-                zmc_zexp2(e, fa, fb);
+                zmc_zexp2<CHK>(e, fa, fb);
             } else {      /* packed map and quadratic form, scalar polynomial: fewer live registers at high D */
-                fa = zmc_zexp_value(zmc_lo(e));
-                fb = zmc_zexp_value(zmc_hi(e));
+                fa = zmc_zexp_value<CHK>(zmc_lo(e));
+                fb = zmc_zexp_value<CHK>(zmc_hi(e));
             }
         }
     }
@@ -487,6 +523,9 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
         unp = a.ppi;
     }
 
+    static constexpr bool HAS_RANGE_PROOF = false;
+    static constexpr bool in_range = false;
+    template <bool CHK = true>
     __device__ __forceinline__ double eval(const zu32* w, double* xout) const {
         double x[D_];
 #pragma unroll
@@ -524,15 +563,31 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
         return 0.0;
     }
     static constexpr bool HAS_PACKED = false;   /* there is no packed FP64 */
+    template <bool CHK = true>
     __device__ __forceinline__ void eval2(const zu32* wa, const zu32* wb, double& fa, double& fb) const {
-        fa = eval(wa, nullptr);
-        fb = eval(wb, nullptr);
+        fa = eval<CHK>(wa, nullptr);
+        fb = eval<CHK>(wb, nullptr);
     }
 };
 
 /* ------------------------------------------------------------------ work-item decoding (R2) */
 /* item -> (cell, trial, chunk); cell -> (parent G, child j); child j -> digits j_d (axis 0 least
  * significant), I'_d = I_d*g + j_d ; path P' = P*k + j (80 bits). */
+/* n = q*d + r. Work-item indices and child indices are below 2^32 except on the very largest levels: the 32-bit division is
+ * ~15 inline instructions, the 64-bit one a subroutine call of ~100 -- and there are 3 + D of them per work item. */
+template <bool FAST>
+__device__ __forceinline__ void zmc_divmod(zu64 n, zu32 d, zu64& q, zu32& r) {
+    if (FAST && (n >> 32) == 0ull) {
+        const zu32 q32 = (zu32)n / d;
+        r = (zu32)n - q32 * d;
+        q = q32;
+    } else {
+        const zu64 q64 = n / d;
+        r = (zu32)(n - q64 * d);
+        q = q64;
+    }
+}
+
 template <int D>
 struct ZmcUnit {
     zu32 inst, trial, chunk;
@@ -540,13 +595,21 @@ struct ZmcUnit {
     zu64 path_lo;
     zu32 path_hi;
     zu32 coords[D];
-    __device__ __forceinline__ void decode(const ZmcSampleArgs& a, zu64 item, zu32 n_chunks) {
-        const zu64 unit = item / n_chunks;
-        chunk = (zu32)(item - unit * n_chunks);
-        cell = unit / a.T;
-        trial = (zu32)(unit - cell * a.T);
-        const zu64 G = cell / a.k;
-        zu64 j = cell - G * a.k;
+    template <bool FAST>
+    __device__ __forceinline__ void decode(const ZmcSampleArgs& a, zu64 item, zu32 n_chunks, zu32 trials_per_item) {
+        zu64 unit;
+        zmc_divmod<FAST>(item, n_chunks, unit, chunk);
+        if (trials_per_item == 1u) zmc_divmod<FAST>(unit, a.T, cell, trial);
+        else { cell = unit; trial = 0u; }       /* the item is the whole cell: trials 0 .. T-1 */
+        zu64 G, j;
+        if (FAST && ((cell | a.k) >> 32) == 0ull) {     /* the usual case, without the 64-bit division routine */
+            const zu32 G32 = (zu32)cell / (zu32)a.k;
+            G = G32;
+            j = (zu32)cell - G32 * (zu32)a.k;
+        } else {
+            G = cell / a.k;
+            j = cell - G * a.k;
+        }
         inst = a.par_inst[G];
         const zu64 plo = a.par_plo[G];
         const zu32 phi = a.par_phi[G];
@@ -555,9 +618,8 @@ struct ZmcUnit {
         path_hi = (zu32)((zu64)phi * a.k + carry);
 #pragma unroll
         for (int d = 0; d < D; ++d) {
-            const zu64 jq = j / a.g;
-            const zu32 jd = (zu32)(j - jq * a.g);
-            j = jq;
+            zu32 jd;
+            zmc_divmod<FAST>(j, a.g, j, jd);
             coords[d] = a.par_coord[(zu64)d * a.par_stride + G] * a.g + jd;
         }
     }
@@ -580,7 +642,16 @@ template <int D> struct ZmcGroup {
  *   MINB    resident CTAs per SM asked of __launch_bounds__ (register cap)
  *   P0_ADD  first-round products M0*q of a group's later calls by 64-bit addition (ALU pipe) instead of IMAD.WIDE
  *   P0_CARRY  ... and the group's own first product as a 64-bit induction variable of the sample loop:
- *           no first-round multiply at all on the FMA-heavy pipe */
+ *           no first-round multiply at all on the FMA-heavy pipe
+ *   FAST_DECODE  32-bit divisions in the item decoding where the operands allow (neutral in time, fewer instructions)
+ *   TRIAL_LOOP   the kernel honours ZmcLevelInfo::trials_per_item (one item = all T trials of a cell; decoding, geometry and the
+ *           latency chain atomic -> parent record -> key/parameters once per cell): +3 % at D = 4, N = 4096; +4.6 % at D = 3,
+ *           N = 2000; +1 % at D = 12; nothing at N >= 1e5. Off: every item is one (cell, trial, chunk) unit
+ *           (profiles/r2_variants.md) */
+/* which kernels loop over the trials of a cell (TRIAL_LOOP below); the host asks too: it plans trials_per_item accordingly.
+ * At D = 6 the loop costs 30 registers (118 -> 148: 3 CTAs per SM instead of 4) and 2 % at N = 1e5. */
+__host__ __device__ constexpr bool zmc_tune_trial_loop(int D) { return D != 6; }
+
 template <class F>
 struct ZmcTune {
     static constexpr int D = F::D;
@@ -602,6 +673,13 @@ struct ZmcTune {
     static constexpr bool P0_CARRY = P0_ADD;
     static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && D >= 7) ? 2 : 3;   /* FP64 at high D spills below 255 registers */
 #endif
+#ifdef ZMC_TUNE_ITEM      /* bit 0: FAST_DECODE, bit 1: TRIAL_LOOP */
+    static constexpr bool FAST_DECODE = (ZMC_TUNE_ITEM & 1) != 0;
+    static constexpr bool TRIAL_LOOP = (ZMC_TUNE_ITEM & 2) != 0;
+#else
+    static constexpr bool FAST_DECODE = true;
+    static constexpr bool TRIAL_LOOP = zmc_tune_trial_loop(D);
+#endif
 };
 
 /* R13: q + f*f. FP32-mode values have 24 significant bits, so the product is exact and one DFMA is the
@@ -611,7 +689,7 @@ __device__ __forceinline__ double zmc_sq_add(double q, double f) {
     return (F::PREC == ZMC_PREC_F32) ? __fma_rn(f, f, q) : __dadd_rn(q, __dmul_rn(f, f));
 }
 
-template <class F, bool SQ>
+template <class F, bool SQ, bool CHK = true>
 __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
                                                double* acc, double* accq, zu64 pg = 0ull, bool have_pg = false) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
@@ -629,7 +707,7 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
 #pragma unroll
         for (int s = 0; s < SG; s += 2) {
             double fa, fb;
-            f.eval2(&w[s * D], &w[(s + 1) * D], fa, fb);
+            f.template eval2<CHK>(&w[s * D], &w[(s + 1) * D], fa, fb);
             acc[s] = __dadd_rn(acc[s], fa);
             acc[s + 1] = __dadd_rn(acc[s + 1], fb);
             if (SQ) { accq[0] = zmc_sq_add<F>(accq[0], fa); accq[1] = zmc_sq_add<F>(accq[1], fb); }
@@ -637,7 +715,7 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
     } else {
 #pragma unroll
         for (int s = 0; s < SG; ++s) {
-            const double fv = f.eval(&w[s * D], nullptr);
+            const double fv = f.template eval<CHK>(&w[s * D], nullptr);
             acc[s] = __dadd_rn(acc[s], fv);
             if (SQ) accq[s & 1] = zmc_sq_add<F>(accq[s & 1], fv);
         }
@@ -645,7 +723,7 @@ __device__ __forceinline__ void zmc_group_eval(const F& f, const ZmcKeySchedule&
 }
 
 /* groups gi and gj: acc[0..SG) takes gi's samples, acc[SG..2SG) gj's -- the same sums as two zmc_group_eval calls */
-template <class F, bool SQ>
+template <class F, bool SQ, bool CHK = true>
 __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi,
                                                     zu32 gj, double* acc, double* accq, zu64 pg = 0ull, bool have_pg = false) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
@@ -665,15 +743,87 @@ __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySche
             for (int c = 0; c < CG; ++c) zmc_philox(gj * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &wb[4 * c]);
         }
         double fa, fb;
-        f.eval2(wa, wb, fa, fb);
+        f.template eval2<CHK>(wa, wb, fa, fb);
         acc[0] = __dadd_rn(acc[0], fa);
         acc[1] = __dadd_rn(acc[1], fb);
         if (SQ) { accq[0] = zmc_sq_add<F>(accq[0], fa); accq[1] = zmc_sq_add<F>(accq[1], fb); }
     } else {
         /* gj = gi + 32: its first product is gi's plus 32*CG*M0 */
-        zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq, pg, have_pg);
-        zmc_group_eval<F, SQ>(f, ks, uc, gj, acc + SG, accq + 2, pg + (zu64)(32 * CG) * (zu64)ZMC_PHILOX_M0, have_pg);
+        zmc_group_eval<F, SQ, CHK>(f, ks, uc, gi, acc, accq, pg, have_pg);
+        zmc_group_eval<F, SQ, CHK>(f, ks, uc, gj, acc + SG, accq + 2, pg + (zu64)(32 * CG) * (zu64)ZMC_PHILOX_M0, have_pg);
     }
+}
+
+/* One lane's share of a work item: the full sample groups gi, gi + 32, ... < gfe. acc[0..SG) sums the groups at even
+ * multiples of 32 from the lane's first one, acc[SG..2SG) those at odd multiples -- whatever UNROLL is. */
+template <class F, bool SQ, bool CHK>
+__device__ __forceinline__ void zmc_full_groups(const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc, zu32 gi, zu32 gfe,
+                                                double* acc, double* accq) {
+    constexpr int CG = ZmcGroup<F::D>::CG;
+    constexpr bool CARRY = ZmcTune<F>::P0_CARRY;     /* the group's first product as a 64-bit induction variable */
+    zu64 pg = (zu64)(gi * (zu32)CG) * (zu64)ZMC_PHILOX_M0;
+    if (ZmcTune<F>::UNROLL == 8) {
+        for (; gi + 224u < gfe; gi += 256u) {
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                zmc_group_eval_pair<F, SQ, CHK>(f, ks, uc, gi + 64u * h, gi + 64u * h + 32u, acc, accq, pg + (zu64)(64 * h * CG) * (zu64)ZMC_PHILOX_M0, CARRY);
+            pg += (zu64)(256 * CG) * (zu64)ZMC_PHILOX_M0;
+        }
+    }
+    if (ZmcTune<F>::UNROLL >= 4) {
+        for (; gi + 96u < gfe; gi += 128u) {
+            zmc_group_eval_pair<F, SQ, CHK>(f, ks, uc, gi, gi + 32u, acc, accq, pg, CARRY);
+            zmc_group_eval_pair<F, SQ, CHK>(f, ks, uc, gi + 64u, gi + 96u, acc, accq, pg + (zu64)(64 * CG) * (zu64)ZMC_PHILOX_M0, CARRY);
+            pg += (zu64)(128 * CG) * (zu64)ZMC_PHILOX_M0;
+        }
+    }
+    for (; gi + 32u < gfe; gi += 64u) {
+        zmc_group_eval_pair<F, SQ, CHK>(f, ks, uc, gi, gi + 32u, acc, accq, pg, CARRY);
+        pg += (zu64)(64 * CG) * (zu64)ZMC_PHILOX_M0;
+    }
+    if (gi < gfe) zmc_group_eval<F, SQ, CHK>(f, ks, uc, gi, acc, accq);
+}
+
+/* One (cell, trial, chunk) unit: the warp's lanes stride over the chunk's sample groups [gb, ge), lane 0 takes the ragged tail,
+ * a shuffle reduction, one 8-byte store (two with SQ). */
+template <class F, bool SQ>
+__device__ __forceinline__ void zmc_unit(const ZmcSampleArgs& a, const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc,
+                                         zu32 lane, zu32 gb, zu32 ge, zu32 gfe, zu32 full_groups, zu32 tail, zu64 out) {
+    constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
+    /* acc[0..SG) sums the groups at even multiples of 32 from the lane's first one, acc[SG..2SG) those at odd multiples --
+     * whatever UNROLL is, so results do not depend on it */
+    double acc[2 * SG], accq[4];     /* sums of squares: two accumulators per group in flight are enough */
+#pragma unroll
+    for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
+    accq[0] = accq[1] = accq[2] = accq[3] = 0.0;
+    /* EXP_QUAD with a range proof for this cell: the loop without zexp's per-sample range test; else the tested loop */
+    if (F::HAS_RANGE_PROOF && f.in_range) zmc_full_groups<F, SQ, false>(f, ks, uc, gb + lane, gfe, acc, accq);
+    else zmc_full_groups<F, SQ, true>(f, ks, uc, gb + lane, gfe, acc, accq);
+    if (tail != 0u && ge > full_groups && lane == 0u) {   /* the partial group: only its first `tail` samples exist */
+        zu32 w[4 * CG];
+        const zu32 q0 = full_groups * (zu32)CG;
+#pragma unroll
+        for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+#pragma unroll
+        for (int s = 0; s < SG; ++s)
+            if ((zu32)s < tail) {
+                const double fv = f.eval(&w[s * D], nullptr);
+                acc[s] = __dadd_rn(acc[s], fv);
+                if (SQ) accq[s & 1] = zmc_sq_add<F>(accq[s & 1], fv);
+            }
+    }
+    double sum = acc[0];
+#pragma unroll
+    for (int s = 1; s < 2 * SG; ++s) sum = __dadd_rn(sum, acc[s]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
+    if (SQ) {
+        double sq = __dadd_rn(__dadd_rn(accq[0], accq[1]), __dadd_rn(accq[2], accq[3]));
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) sq = __dadd_rn(sq, __shfl_down_sync(0xFFFFFFFFu, sq, off));
+        if (lane == 0u) a.partial_q[out] = sq;
+    }
+    if (lane == 0u) a.partial[out] = sum;
 }
 
 /* UKEY: every work item has the same Philox key (n_instances == 1); it comes from the kernel
@@ -682,7 +832,7 @@ __device__ __forceinline__ void zmc_group_eval_pair(const F& f, const ZmcKeySche
 /* SQ (R13): also sum f^2 per unit, into partial_q. */
 template <class F, bool UKEY, bool SQ = false>
 __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
-    constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
+    constexpr int D = F::D, SG = ZmcGroup<D>::SG;
     const zu32 lane = threadIdx.x & 31u;
     ZmcLevelInfo* const info = a.info;
     const zu64 n_items = info->n_items;
@@ -691,6 +841,7 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
     const zu32 full_groups = (zu32)(a.N / (zu64)SG);       /* groups whose SG samples all exist */
     const zu32 tail = (zu32)(a.N - (zu64)full_groups * SG); /* samples in the last, partial group */
     const zu32 n_groups = full_groups + (tail ? 1u : 0u);
+    const zu32 tpi = ZmcTune<F>::TRIAL_LOOP ? info->trials_per_item : 1u;
 
     for (;;) {
         zu64 item = 0;
@@ -699,14 +850,12 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
         if (item >= n_items) break;
 
         ZmcUnit<D> u;
-        u.decode(a, item, n_chunks);
+        u.template decode<ZmcTune<F>::FAST_DECODE>(a, item, n_chunks, tpi);
         F f;
         f.setup(a, u.inst, u.coords);
         ZmcKeySchedule ks;
         if (UKEY) ks.init(a.ukey[0], a.ukey[1]);
         else ks.init(a.keys[2 * u.inst], a.keys[2 * u.inst + 1]);
-        ZmcUnitCounter uc;
-        uc.init(u.path_lo, u.path_hi, a.level, u.trial);
 
         /* a chunk before the last ends where the next begins ((chunk + 1) * chunk_groups <= (n_chunks - 1) * chunk_groups < n_groups);
          * the last ends with the unit. No sum that could pass 2^32, and -- measured -- the form ptxas schedules best:
@@ -715,52 +864,22 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
         const zu32 ge = (u.chunk + 1u < n_chunks) ? gb + chunk_groups : n_groups;
         const zu32 gfe = (ge < full_groups) ? ge : full_groups;
 
-        /* lanes stride over the chunk's groups; acc[0..SG) sums the groups at even multiples of 32 from the
-         * lane's first one, acc[SG..2SG) those at odd multiples -- whatever UNROLL is, so results do not depend on it */
-        double acc[2 * SG], accq[4];     /* sums of squares: two accumulators per group in flight are enough */
-#pragma unroll
-        for (int s = 0; s < 2 * SG; ++s) acc[s] = 0.0;
-        accq[0] = accq[1] = accq[2] = accq[3] = 0.0;
-        zu32 gi = gb + lane;
-        constexpr bool CARRY = ZmcTune<F>::P0_CARRY;     /* the group's first product as a 64-bit induction variable */
-        zu64 pg = (zu64)(gi * (zu32)CG) * (zu64)ZMC_PHILOX_M0;
-        if (ZmcTune<F>::UNROLL == 4) {
-            for (; gi + 96u < gfe; gi += 128u) {
-                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq, pg, CARRY);
-                zmc_group_eval_pair<F, SQ>(f, ks, uc, gi + 64u, gi + 96u, acc, accq, pg + (zu64)(64 * CG) * (zu64)ZMC_PHILOX_M0, CARRY);
-                pg += (zu64)(128 * CG) * (zu64)ZMC_PHILOX_M0;
+        if (!ZmcTune<F>::TRIAL_LOOP) {          /* the item is one unit */
+            ZmcUnitCounter uc;
+            uc.init(u.path_lo, u.path_hi, a.level, u.trial);
+            zmc_unit<F, SQ>(a, f, ks, uc, lane, gb, ge, gfe, full_groups, tail, item);
+        } else {
+            /* the item's units: one, or -- trials_per_item == T -- the T trials of the cell, which share everything above */
+            zu64 out = (u.cell * (zu64)a.T + u.trial) * n_chunks + u.chunk;     /* = item when trials_per_item == 1 */
+            for (zu32 trial = u.trial; trial < u.trial + tpi; ++trial, ++out) {
+                ZmcUnitCounter uc;
+                uc.init(u.path_lo, u.path_hi, a.level, trial);
+                /* opaque to the optimiser: otherwise ptxas hoists the per-cell halves of the first Philox rounds above this loop
+                 * and takes 8 more registers at D = 6 */
+                asm volatile("" : "+r"(uc.c1), "+r"(uc.c2), "+r"(uc.c3));
+                zmc_unit<F, SQ>(a, f, ks, uc, lane, gb, ge, gfe, full_groups, tail, out);
             }
         }
-        for (; gi + 32u < gfe; gi += 64u) {
-            zmc_group_eval_pair<F, SQ>(f, ks, uc, gi, gi + 32u, acc, accq, pg, CARRY);
-            pg += (zu64)(64 * CG) * (zu64)ZMC_PHILOX_M0;
-        }
-        if (gi < gfe) zmc_group_eval<F, SQ>(f, ks, uc, gi, acc, accq);
-        if (tail != 0u && ge > full_groups && lane == 0u) {   /* the partial group: only its first `tail` samples exist */
-            zu32 w[4 * CG];
-            const zu32 q0 = full_groups * (zu32)CG;
-#pragma unroll
-            for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
-#pragma unroll
-            for (int s = 0; s < SG; ++s)
-                if ((zu32)s < tail) {
-                    const double fv = f.eval(&w[s * D], nullptr);
-                    acc[s] = __dadd_rn(acc[s], fv);
-                    if (SQ) accq[s & 1] = zmc_sq_add<F>(accq[s & 1], fv);
-                }
-        }
-        double sum = acc[0];
-#pragma unroll
-        for (int s = 1; s < 2 * SG; ++s) sum = __dadd_rn(sum, acc[s]);
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
-        if (SQ) {
-            double sq = __dadd_rn(__dadd_rn(accq[0], accq[1]), __dadd_rn(accq[2], accq[3]));
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) sq = __dadd_rn(sq, __shfl_down_sync(0xFFFFFFFFu, sq, off));
-            if (lane == 0u) a.partial_q[item] = sq;
-        }
-        if (lane == 0u) a.partial[item] = sum;
     }
 }
 

@@ -1,11 +1,38 @@
-"""Issue-rate microbenchmarks of the pipes the sampling kernel uses (zmc_microbench in include/zmc.h).
+"""Issue-rate microbenchmarks of the pipes the sampling kernel uses (csrc/zmc_microbench.cu, built as its own
+library libzmc_microbench.so by build.build_microbench(); a measurement tool, not part of the product ABI).
 
     python -m paper_1902_07916_b200.microbench            # prints a markdown table (needs a B200)
 
 They give the denominator of the ALU roofline: warp-instructions per SM per clock
 for IMAD.WIDE.U32, LOP3, FFMA, ... and whole Philox4x32-10 calls.
 """
-from . import binding as B
+import ctypes as C
+
+from . import build as _build
+
+_lib = None
+
+
+class MicrobenchError(RuntimeError):
+    def __init__(self, status):
+        super().__init__("zmc_microbench status %d" % status)
+        self.status = status
+
+
+def microbench(which: int, stream: int = 0):
+    """which: 0 IMAD.WIDE.U32, 1 LOP3, 2 IMAD.WIDE+LOP3, 3 FFMA, 4 FADD, 5 DADD, 6 F2F pair, 7 MUFU.SIN, 8 MUFU.EX2, 9 DFMA,
+    10 Philox4x32-10 calls, 11 I2F/F2I pair, 12 LEA.HI, 13 IMAD lo, 14 IMAD.HI, 15 64-bit add, 16 IMAD.WIDE by a register;
+    100 + 10*X + j: Philox calls each followed by K = (0, 10, 20, 40)[j] extra instructions of kind X (see MIX).
+    Returns (warp-instructions per SM per clock, SM MHz seen)."""
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build_microbench())
+        _lib.zmc_microbench.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    r, mhz = C.c_double(), C.c_double()
+    rc = _lib.zmc_microbench(which, C.c_void_p(stream), C.byref(r), C.byref(mhz))
+    if rc != 0:
+        raise MicrobenchError(rc)
+    return r.value, mhz.value
 
 NAMES = {0: "IMAD.WIDE.U32", 1: "LOP3", 2: "IMAD.WIDE.U32 + LOP3 (Philox round mix)", 3: "FFMA", 4: "FADD", 5: "DADD",
          6: "F2F.F64.F32 + F2F.F32.F64 (dependent pair, per instruction)", 7: "MUFU.SIN", 8: "MUFU.EX2", 9: "DFMA", 10: "Philox4x32-10 calls (x32 lanes)",
@@ -18,8 +45,8 @@ def main():
     print("|---|---|---|---|---|")
     for w in sorted(NAMES):
         try:
-            r, mhz = B.microbench(w)
-        except B.ZmcError as e:
+            r, mhz = microbench(w)
+        except MicrobenchError as e:
             print("| %d | %s | error %d | | |" % (w, NAMES[w], e.status))
             continue
         print("| %d | %s | %.3f | %.2f | %.0f |" % (w, NAMES[w], r, 4.0 / r if r > 0 else float("nan"), mhz))
@@ -38,7 +65,7 @@ def mix_table():
     for x in sorted(MIX):
         clk = []
         for j, k in enumerate(MIX_K):
-            r, _ = B.microbench(100 + 10 * x + j)
+            r, _ = microbench(100 + 10 * x + j)
             clk.append(4.0 / r)
         print("| %s | " % MIX[x] + " | ".join("%.1f" % c for c in clk) + " | %.2f |" % ((clk[-1] - clk[0]) / MIX_K[-1]))
 

@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "slow: many GPU-minutes; skipped unless ZMC_RUN_SLOW=1 (tests/test_gpu_slow.py)")
 
 
 def pytest_collection_modifyitems(config, items):

@@ -8,18 +8,8 @@ import numpy as np
 import oracle as O
 from paper_1902_07916_b200 import workloads as W
 
-_ORC_INTEGRAND = {W.CONST: O.CONST, W.LINEAR: O.LINEAR, W.SIN_SUM: O.SIN_SUM, W.EXP_QUAD: O.EXP_QUAD}
-_ORC_PRECISION = {W.F64: O.F64, W.F32: O.F32}
-
-
 def oracle_config(w: W.Workload, **over) -> O.Config:
-    cfg = O.Config(dim=w.dim, lower=list(w.lower), upper=list(w.upper), g=w.g, n_samples=w.n_samples,
-                   trials=w.trials, depth=w.depth, sigma_multiplier=w.sigma_multiplier, seed=w.seed,
-                   integrand=_ORC_INTEGRAND[w.integrand], precision=_ORC_PRECISION[w.precision],
-                   params=w.params, n_instances=w.n_instances, max_groups_per_level=w.max_groups_per_level)
-    for k, v in over.items():
-        setattr(cfg, k, v)
-    return cfg
+    return O.config_from_workload(w, **over)
 
 
 def closed_sin_sum(lower, upper) -> float:
@@ -96,7 +86,7 @@ def compare_tree(it, ores, w: W.Workload, *, tol_sum=1e-12, tol_stat=1e-11, exac
         # tau = mean(s) + m*pstd(s) is (1 + |m|)-Lipschitz in max|ds|: where s itself is ill-conditioned (cells so small that
         # f is constant to 9 digits) the thresholds inherit exactly that much and no more
         ds = float(np.abs(gl.s - ol.s).max())
-        assert np.abs(gl.tau - ol.tau).max() <= 100 * tol_stat * max(ol.tau.max(), 1e-300) + (1.0 + abs(w.sigma_multiplier)) * ds
+        assert np.abs(gl.tau - ol.tau).max() <= 100 * tol_stat * max(np.abs(ol.tau).max(), 1e-300) + (1.0 + abs(w.sigma_multiplier)) * ds      # |tau|: m < 0 makes tau negative
         if exact_sets:
             np.testing.assert_array_equal(gl.refined, ol.refined)
         n_cmp += ol.n_cells

@@ -49,13 +49,12 @@ def test_create_validates_arguments():
     dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
 
     def create(dim=3, lower=lo, upper=up, g=4, N=100, T=5, depth=2, m=1.5, seed=1):
-        h = C.c_void_p()
+        h = C.c_void_p(0xDEAD)     # a failed zmc_create must overwrite this with NULL: there is nothing to destroy
         rc = L.zmc_create(C.byref(h), dim, dp(lower) if lower is not None else None, dp(upper) if upper is not None else None,
                           g, N, T, depth, m, seed)
-        msg = L.zmc_last_error(h).decode() if h else ""
-        if h:
-            L.zmc_destroy(h)
-        return rc, msg
+        assert rc != B.OK          # every case below is invalid (and without a device even a valid one fails)
+        assert not h, "a failed zmc_create left a context behind"
+        return rc, L.zmc_last_error(None).decode()
 
     assert create(dim=0)[0] == B.ERR_ARG
     assert create(lower=None)[0] == B.ERR_ARG
@@ -70,10 +69,13 @@ def test_create_validates_arguments():
     assert rc == B.ERR_RANGE and "255" in msg
     assert create(depth=16)[0] == B.ERR_RANGE
     assert create(dim=17, lower=np.zeros(17), upper=np.ones(17))[0] == B.ERR_RANGE
-    assert create(N=2 ** 33)[0] == B.ERR_RANGE                          # N*D/4 >= 2^32
+    assert create(N=2 ** 33)[0] == B.ERR_RANGE                          # N*D >= 2^34 - 2^14 (R3)
+    rc, msg = create(dim=1, lower=np.zeros(1), upper=np.ones(1), N=2 ** 34 - 2 ** 14)
+    assert rc == B.ERR_RANGE and "2^34 - 2^14" in msg
     assert create(dim=12, lower=np.zeros(12), upper=np.ones(12), g=4, depth=4)[0] == B.ERR_RANGE   # 96-bit path
     assert create(g=70000, depth=2)[0] == B.ERR_RANGE                   # g^depth > 2^32
     assert L.zmc_create(None, 3, dp(lo), dp(up), 4, 100, 5, 2, 1.5, 1) == B.ERR_ARG
+    assert L.zmc_last_error(None).decode() == "out is null"
     assert L.zmc_status_string(B.ERR_CAPACITY).decode() == "level capacity exceeded"
 
 
@@ -83,8 +85,7 @@ def test_no_device_means_error_not_fallback():
         pytest.skip("a CUDA device is present")
     with pytest.raises(B.ZmcError) as e:
         B.Integrator(3, [0.0] * 3, [1.0] * 3, 4, 100, 5, 2, 1.5, 1)
-    assert e.value.status == B.ERR_CUDA
-    assert B.lib().zmc_microbench(0, None, None, None) == B.ERR_CUDA
+    assert e.value.status == B.ERR_CUDA and "no CUDA device" in str(e.value)
 
 
 def test_headline_kernels_keep_their_register_budget():
@@ -142,3 +143,44 @@ def test_binding_constants_match_the_header():
         subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), "-o", os.path.join(d, "s"), os.path.join(d, "s.c")], check=True)
         a, b = subprocess.run([os.path.join(d, "s")], capture_output=True, text=True, check=True).stdout.split()
     assert int(a) == C.sizeof(B.LevelStats) and int(b) == C.sizeof(B.Stats)
+
+
+def test_failed_create_from_c_leaves_nothing_to_destroy():
+    """The contract of include/zmc.h as a C caller sees it: a failed zmc_create sets *out to NULL, the reason is
+    zmc_last_error(NULL), zmc_destroy(NULL) is a no-op, and every other call refuses a NULL context."""
+    src = r"""
+#include <stdio.h>
+#include <string.h>
+#include "zmc.h"
+int main(void) {
+    double lo[3] = {0, 0, 0}, up[3] = {1, 1, 1}, bad_up[3] = {1, 0, 1};
+    zmc_ctx* c = (zmc_ctx*)0x1;
+    int rc = zmc_create(&c, 3, lo, bad_up, 4, 100, 5, 2, 1.5, 1);
+    if (rc != ZMC_ERR_ARG || c != NULL) { printf("bounds: rc %d ctx %p\n", rc, (void*)c); return 1; }
+    if (strstr(zmc_last_error(NULL), "upper > lower") == NULL) { printf("message: %s\n", zmc_last_error(NULL)); return 2; }
+    c = (zmc_ctx*)0x1;
+    rc = zmc_create(&c, 3, lo, up, 4, 100, 300, 2, 1.5, 1);
+    if (rc != ZMC_ERR_RANGE || c != NULL) { printf("trials: rc %d ctx %p\n", rc, (void*)c); return 3; }
+    zmc_destroy(c);   /* NULL: no-op */
+    if (zmc_run(NULL, NULL) != ZMC_ERR_ARG || zmc_set_option(NULL, ZMC_OPT_PRECISION, ZMC_F32) != ZMC_ERR_ARG) return 4;
+    double v, s;
+    if (zmc_result(NULL, &v, &s) != ZMC_ERR_ARG) return 5;
+    printf("ok\n");
+    return 0;
+}
+"""
+    import tempfile
+    B.lib()
+    with tempfile.TemporaryDirectory() as d:
+        open(os.path.join(d, "t.c"), "w").write(src)
+        exe = os.path.join(d, "t")
+        subprocess.run(["gcc", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-o", exe, os.path.join(d, "t.c"),
+                        B.LIB_PATH, "-Wl,-rpath," + os.path.dirname(B.LIB_PATH)], check=True)
+        r = subprocess.run([exe], capture_output=True, text=True)
+    assert r.returncode == 0 and r.stdout.strip() == "ok", (r.returncode, r.stdout, r.stderr)
+
+
+def test_microbench_is_not_part_of_the_product_library():
+    syms = subprocess.run(["nm", "-D", "--defined-only", B.LIB_PATH], capture_output=True, text=True).stdout
+    assert "zmc_microbench" not in syms
+    assert "zmc_microbench" not in open(os.path.join(ROOT, "include", "zmc.h")).read()
