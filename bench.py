@@ -110,11 +110,6 @@ def traffic_from_profiles(workload, math):
     return sum(vals) / len(vals) if vals else None
 
 
-def launches_per_step(depth, by_spread=False):
-    return 1 + (9 if by_spread else 6) * depth + 1     # init ; per level: sample, cell_stats, threshold, scan, scatter, accumulate ; finalize
-                                 # (zmc_keys_kernel runs once per context, with the parameter upload)
-
-
 class ClockSampler:
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
@@ -368,7 +363,7 @@ def main():
                        "deviation": DEVIATIONS.get(args.workload)},
             "result": {"value": float(value_v[0]), "std": float(value_s[0])},
             "wall_ms_per_step": 1e3 * t_wall / args.steps,
-            "gpu_launches": launches_per_step(w.depth, order == B.BUDGET_LARGEST_SPREAD and w.max_groups_per_level > 0) * args.steps,
+            "gpu_launches": int(st.kernel_launches) * args.steps,      # counted by zmc_run as it enqueues them; all the library's own
             "roofline": roofline}
     if clocks is not None:
         line["clocks"] = clocks

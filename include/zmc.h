@@ -159,6 +159,7 @@ typedef struct zmc_stats_t {
     int32_t grid_blocks, block_threads;
     int32_t kernel_origin;          /* sampling kernel: 0 pre-compiled, 1 compiled by NVRTC for this context, 2 from the process-wide
                                        cache, 3 from the on-disk cache (ZMC_CACHE_DIR) */
+    int32_t kernel_launches;        /* kernels the last zmc_run enqueued (all the library's own; a CUDA graph replays the same nodes) */
     zmc_level_stats level[ZMC_MAX_DEPTH];
 } zmc_stats_t;
 

@@ -47,7 +47,7 @@ class Stats(C.Structure):
     _fields_ = [("levels", C.c_int32), ("overflow", C.c_int32), ("nonfinite", C.c_uint64),
                 ("total_evals", C.c_uint64), ("total_ms", C.c_float), ("regs_per_thread", C.c_int32),
                 ("grid_blocks", C.c_int32), ("block_threads", C.c_int32), ("kernel_origin", C.c_int32),
-                ("level", LevelStats * MAX_DEPTH)]
+                ("kernel_launches", C.c_int32), ("level", LevelStats * MAX_DEPTH)]
 
 
 class ZmcError(RuntimeError):

@@ -24,6 +24,11 @@
 
 #define ZMC_CTL_THREADS 256
 #define ZMC_SCAN_THREADS 1024
+/* A sibling group of k cells is handled as ceil(k / ZMC_TILE_CELLS) tiles of consecutive cells, one CTA per tile, so that a level
+ * that is ONE group of 10^5 .. 10^6 cells (BASELINE.json configs[4]; the paper's Table 3 and 4 sizes) is not walked by one CTA.
+ * Groups up to ZMC_TILE_CELLS cells are one tile and take the single-launch threshold kernel. The tiling depends on k only, so
+ * the reductions keep a fixed shape: repeated runs and different grid sizes give identical bits. */
+#define ZMC_TILE_CELLS 4096
 
 struct ZmcParents {
     zu32* inst;
@@ -44,6 +49,9 @@ struct ZmcCtlArgs {
     double m;               /* sigma multiplier */
     zu64 budget;            /* R12; ~0 = off */
     zu64 cap_par;           /* capacity of a parent list */
+    zu32 tpg;               /* tiles per sibling group = ceil(k / ZMC_TILE_CELLS): the unit of the flag/compaction kernels */
+    double* tsum;           /* [tile] sum of s            (tpg > 1 only: the three passes of R6 are three launches) */
+    double* tsq;            /* [tile] sum of (s - mean)^2 (tpg > 1 only) */
     ZmcParents cur, next;
     zu64 par_stride;
     const double* params;
@@ -55,11 +63,11 @@ struct ZmcCtlArgs {
     double* s;              /* [cell] */
     unsigned char* refined; /* [cell], or nullptr */
     double* tau;            /* [group] */
-    zu64* cnt;              /* [group] flagged cells */
-    zu64* excl;             /* [group] exclusive prefix of cnt over all groups */
-    double* gacc;           /* [group][2] accepted (sum mu, sum s^2) */
-    zu64* gfirst;           /* [instance] first group */
-    zu64* gend;             /* [instance] one past the last group */
+    zu64* cnt;              /* [tile] flagged cells */
+    zu64* excl;             /* [tile] exclusive prefix of cnt over all tiles */
+    double* gacc;           /* [tile][2] accepted (sum mu, sum s^2) */
+    zu64* gfirst;           /* [instance] first tile */
+    zu64* gend;             /* [instance] one past the last tile */
     zu64* out0;             /* [instance] first output slot */
     double* value;          /* [instance] */
     double* var;            /* [instance] */
@@ -73,9 +81,9 @@ struct ZmcCtlArgs {
     zu32 budget_order;      /* 0: first B flagged cells in path order (R12) ; 1: the B largest spreads */
     zu64* piv;              /* [instance] key (bits of s) of the B-th largest flagged spread; 0 with quota ~0 = keep every flagged cell */
     zu64* quota;            /* [instance] how many cells with s == pivot are kept (the first in path order) */
-    zu64* cnt_gt;           /* [group] flagged cells with key > pivot */
-    zu64* cnt_eq;           /* [group] flagged cells with key == pivot */
-    zu64* excl_gt;          /* [group] exclusive prefixes over all groups */
+    zu64* cnt_gt;           /* [tile] flagged cells with key > pivot */
+    zu64* cnt_eq;           /* [tile] flagged cells with key == pivot */
+    zu64* excl_gt;          /* [tile] exclusive prefixes over all tiles */
     zu64* excl_eq;
 };
 
@@ -225,8 +233,20 @@ __device__ __forceinline__ zu64 zmc_block_sum_u64(zu64 v, zu64* smem) {
     return smem[0];
 }
 
-/* R6: one block per sibling group; tau = mean(s) + m * pstd(s), both moments two-pass, population
- * form ("the mean and standard deviation of the calculated k standard deviations").
+/* tile -> its sibling group and cell range */
+struct ZmcTile {
+    zu64 G, c0, c1;
+    __device__ __forceinline__ ZmcTile(const ZmcCtlArgs& c, zu64 tile) {
+        G = tile / c.tpg;
+        const zu64 t = tile - G * c.tpg;
+        c0 = G * c.k + t * (zu64)ZMC_TILE_CELLS;
+        const zu64 end = (G + 1ull) * c.k;
+        c1 = (c0 + (zu64)ZMC_TILE_CELLS < end) ? c0 + (zu64)ZMC_TILE_CELLS : end;
+    }
+};
+
+/* R6: one block per sibling group of at most ZMC_TILE_CELLS cells (tpg == 1); tau = mean(s) + m * pstd(s), both moments
+ * two-pass, population form ("the mean and standard deviation of the calculated k standard deviations").
  * R7: flagged iff level < L and s > tau (strict; NaN compares false). */
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
@@ -250,6 +270,49 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __
             for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) n += (s[j] > tau) ? 1ull : 0ull;
         n = zmc_block_sum_u64(n, smem_u);
         if (threadIdx.x == 0) { c.tau[G] = tau; c.cnt[G] = n; }
+    }
+}
+
+/* R6 for groups of more than ZMC_TILE_CELLS cells (tpg > 1): the same two-pass moments, one block per TILE and one launch per
+ * pass, because each pass needs the whole group's previous one:
+ *   PASS 0  tsum[tile] = sum of s over the tile
+ *   PASS 1  mean_G = (sum of the group's tsum, fixed shape) / k ;  tsq[tile] = sum of (s - mean_G)^2 over the tile
+ *   PASS 2  pstd_G = sqrt((sum of the group's tsq) / k) ; tau_G = mean_G + m * pstd_G ; cnt[tile] = #(s > tau_G) in the tile */
+__device__ __forceinline__ double zmc_group_total(const double* t, zu64 G, zu32 tpg, double* smem) {
+    double part = 0.0;
+    for (zu32 i = threadIdx.x; i < tpg; i += ZMC_CTL_THREADS) part = __dadd_rn(part, t[G * tpg + i]);
+    return zmc_block_sum(part, smem);
+}
+
+template <int PASS>
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_pass_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    __shared__ double smem[ZMC_CTL_THREADS];
+    __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
+    const double dk = (double)c.k;
+    for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const ZmcTile T(c, tile);
+        double mean = 0.0, tau = 0.0;
+        if (PASS >= 1) mean = __ddiv_rn(zmc_group_total(c.tsum, T.G, c.tpg, smem), dk);
+        if (PASS == 2) {
+            const double pstd = __dsqrt_rn(__ddiv_rn(zmc_group_total(c.tsq, T.G, c.tpg, smem), dk));
+            tau = __dadd_rn(mean, __dmul_rn(c.m, pstd));
+        }
+        double part = 0.0;
+        zu64 n = 0;
+        for (zu64 cell = T.c0 + threadIdx.x; cell < T.c1; cell += ZMC_CTL_THREADS) {
+            const double sj = c.s[cell];
+            if (PASS == 0) part = __dadd_rn(part, sj);
+            if (PASS == 1) { const double d = __dadd_rn(sj, -mean); part = __dadd_rn(part, __dmul_rn(d, d)); }
+            if (PASS == 2) n += (c.level < c.L && sj > tau) ? 1ull : 0ull;
+        }
+        if (PASS <= 1) {
+            const double tot = zmc_block_sum(part, smem);
+            if (threadIdx.x == 0) (PASS == 0 ? c.tsum : c.tsq)[tile] = tot;
+        } else {
+            n = zmc_block_sum_u64(n, smem_u);
+            if (threadIdx.x == 0) { c.cnt[tile] = n; if (tile == T.G * c.tpg) c.tau[T.G] = tau; }
+        }
     }
 }
 
@@ -281,26 +344,26 @@ __device__ __forceinline__ zu64 zmc_scan_block_excl(zu64 v, zu64* warp_tot, zu64
     return warp_tot[warp] + inc - v;
 }
 
-/* One block. (A) exclusive scan of cnt over groups and the first/last group of every instance
- * (groups are sorted by instance); (B) per instance: flagged c_b, kept = min(c_b, B) (R12), exclusive
+/* One block. (A) exclusive scan of cnt over the tiles and the first/last tile of every instance
+ * (groups, hence tiles, are sorted by instance); (B) per instance: flagged c_b, kept = min(c_b, B) (R12), exclusive
  * scan -> first output slot; (C) the next level's plan. */
 __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu64 warp_tot[32];
     __shared__ zu64 total;
     __shared__ zu64 carry;
-    const zu64 n_groups = c.info[c.level].n_groups;
+    const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
     for (zu64 b = threadIdx.x; b < c.n_inst; b += ZMC_SCAN_THREADS) { c.gfirst[b] = 0; c.gend[b] = 0; }
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
-    for (zu64 base = 0; base < n_groups; base += ZMC_SCAN_THREADS) {
-        const zu64 G = base + threadIdx.x;
-        const zu64 v = (G < n_groups) ? c.cnt[G] : 0ull;
+    for (zu64 base = 0; base < n_tiles; base += ZMC_SCAN_THREADS) {
+        const zu64 t = base + threadIdx.x;
+        const zu64 v = (t < n_tiles) ? c.cnt[t] : 0ull;
         const zu64 ex = zmc_scan_block_excl(v, warp_tot, &total);
-        if (G < n_groups) {
-            c.excl[G] = carry + ex;
-            const zu32 me = c.cur.inst[G];
-            if (G == 0 || c.cur.inst[G - 1] != me) c.gfirst[me] = G;
-            if (G + 1 == n_groups || c.cur.inst[G + 1] != me) c.gend[me] = G + 1;
+        if (t < n_tiles) {
+            c.excl[t] = carry + ex;
+            const zu32 me = c.cur.inst[t / c.tpg];
+            if (t == 0 || c.cur.inst[(t - 1) / c.tpg] != me) c.gfirst[me] = t;
+            if (t + 1 == n_tiles || c.cur.inst[(t + 1) / c.tpg] != me) c.gend[me] = t + 1;
         }
         __syncthreads();
         if (threadIdx.x == 0) carry += total;
@@ -345,8 +408,9 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __gr
     __shared__ zu32 hist[256];
     __shared__ zu64 sh_prefix, sh_need, sh_above;
     for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
-        const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
+        const zu64 g0 = c.gfirst[b], g1 = c.gend[b];     /* tiles; an instance owns whole groups, i.e. multiples of tpg tiles */
         const zu64 cb = (g1 > g0) ? c.excl[g1 - 1] + c.cnt[g1 - 1] - c.excl[g0] : 0ull;
+        const zu64 cell0 = (g0 / c.tpg) * c.k, cell1 = (g1 / c.tpg) * c.k;
         __syncthreads();
         if (cb <= c.budget) {   /* nothing to cut: every flagged cell is kept -- also those with s == +0 (key 0), flagged when tau < 0 (m < 0) */
             if (threadIdx.x == 0) { c.piv[b] = 0ull; c.quota[b] = ~0ull; }
@@ -358,7 +422,7 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __gr
             for (int i = threadIdx.x; i < 256; i += ZMC_SCAN_THREADS) hist[i] = 0u;
             __syncthreads();
             const zu64 prefix = sh_prefix;
-            for (zu64 cell = g0 * c.k + threadIdx.x; cell < g1 * c.k; cell += ZMC_SCAN_THREADS) {
+            for (zu64 cell = cell0 + threadIdx.x; cell < cell1; cell += ZMC_SCAN_THREADS) {
                 const double sj = c.s[cell];
                 if (sj > c.tau[cell / c.k]) {
                     const zu64 key = (zu64)__double_as_longlong(sj);
@@ -383,34 +447,36 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __gr
     }
 }
 
-/* per sibling group: flagged cells above and at the instance's pivot */
+/* per tile: flagged cells above and at the instance's pivot */
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_count2_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu64 smem_u[ZMC_CTL_THREADS];
-    const zu64 n_groups = c.info[c.level].n_groups;
-    for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
-        const double* s = c.s + G * c.k;
-        const double tau = c.tau[G];
-        const zu64 piv = c.piv[c.cur.inst[G]];
+    const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
+    for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const ZmcTile T(c, tile);
+        const double tau = c.tau[T.G];
+        const zu64 piv = c.piv[c.cur.inst[T.G]];
         zu64 ngt = 0, neq = 0;
         if (c.level < c.L)
-            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS)
-                if (s[j] > tau) {
-                    const zu64 key = (zu64)__double_as_longlong(s[j]);
+            for (zu64 cell = T.c0 + threadIdx.x; cell < T.c1; cell += ZMC_CTL_THREADS) {
+                const double sj = c.s[cell];
+                if (sj > tau) {
+                    const zu64 key = (zu64)__double_as_longlong(sj);
                     ngt += (key > piv) ? 1ull : 0ull;
                     neq += (key == piv) ? 1ull : 0ull;
                 }
+            }
         ngt = zmc_block_sum_u64(ngt, smem_u);
         neq = zmc_block_sum_u64(neq, smem_u);
-        if (threadIdx.x == 0) { c.cnt_gt[G] = ngt; c.cnt_eq[G] = neq; }
+        if (threadIdx.x == 0) { c.cnt_gt[tile] = ngt; c.cnt_eq[tile] = neq; }
     }
 }
 
-/* One block: exclusive scans of cnt_gt and cnt_eq over the groups. */
+/* One block: exclusive scans of cnt_gt and cnt_eq over the tiles. */
 __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu64 warp_tot[32];
     __shared__ zu64 total;
     __shared__ zu64 carry;
-    const zu64 n_groups = c.info[c.level].n_groups;
+    const zu64 n_groups = c.info[c.level].n_groups * c.tpg;     /* tiles */
     for (int which = 0; which < 2; ++which) {
         const zu64* in = which ? c.cnt_eq : c.cnt_gt;
         zu64* out = which ? c.excl_eq : c.excl_gt;
@@ -429,38 +495,43 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __gri
     }
 }
 
-/* R7: one block per sibling group. Flagged cells get their rank within the instance (stable, path
+/* R7: one block per tile. Flagged cells get their rank within the instance (stable, path
  * order); rank < B (R12) and slot < capacity -> the child record (R2) is written to the next parent
- * list. Every other cell is accepted: its mu and s^2 go into the group's fixed-shape sums. */
+ * list. Every other cell is accepted: its mu and s^2 go into the tile's fixed-shape sums. */
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
     __shared__ zu32 warp_cnt[ZMC_CTL_THREADS / 32], warp_cnt_eq[ZMC_CTL_THREADS / 32];
     __shared__ zu64 run, run_eq;
-    const zu64 n_groups = c.info[c.level].n_groups;
+    const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
     const zu32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
+    for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const ZmcTile T(c, tile);
+        const zu64 G = T.G;
         const zu32 inst = c.cur.inst[G];
         const double tau = c.tau[G];
         const bool by_spread = (c.budget_order != 0) && (c.budget != ~0ull);
         const zu64 gf = c.gfirst[inst];
-        const zu64 r0 = c.excl[G] - c.excl[gf];   /* flagged cells of this instance in earlier groups */
-        const zu64 r0_gt = by_spread ? c.excl_gt[G] - c.excl_gt[gf] : 0ull;   /* ... above the pivot */
-        const zu64 r0_eq = by_spread ? c.excl_eq[G] - c.excl_eq[gf] : 0ull;   /* ... at the pivot */
+        const zu64 r0 = c.excl[tile] - c.excl[gf];   /* flagged cells of this instance in earlier tiles */
+        const zu64 r0_gt = by_spread ? c.excl_gt[tile] - c.excl_gt[gf] : 0ull;   /* ... above the pivot */
+        const zu64 r0_eq = by_spread ? c.excl_eq[tile] - c.excl_eq[gf] : 0ull;   /* ... at the pivot */
         const zu64 piv = by_spread ? c.piv[inst] : 0ull;
         const zu64 quota = by_spread ? c.quota[inst] : 0ull;
         const zu64 slot0 = c.out0[inst];
         const zu64 plo = c.cur.plo[G];
         const zu32 phi = c.cur.phi[G];
+        const zu64 j0 = T.c0 - G * c.k;              /* child index of the tile's first cell */
+        const zu64 n_tile = T.c1 - T.c0;
         double acc_mu = 0.0, acc_var = 0.0;
         __syncthreads();
         if (threadIdx.x == 0) { run = 0; run_eq = 0; }
         __syncthreads();
-        for (zu64 base = 0; base < c.k; base += ZMC_CTL_THREADS) {
-            const zu64 j = base + threadIdx.x;
-            const zu64 cell = G * c.k + j;
+        for (zu64 base = 0; base < n_tile; base += ZMC_CTL_THREADS) {
+            const zu64 i = base + threadIdx.x;
+            const zu64 j = j0 + i;
+            const zu64 cell = T.c0 + i;
             double sj = 0.0, muj = 0.0;
             bool flag = false;
-            if (j < c.k) {
+            if (i < n_tile) {
                 sj = c.s[cell];
                 muj = c.mu[cell];
                 flag = (c.level < c.L) && (sj > tau);
@@ -514,7 +585,7 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
                     }
                 }
             }
-            if (j < c.k) {
+            if (i < n_tile) {
                 if (!kept) { acc_mu = __dadd_rn(acc_mu, muj); acc_var = __dadd_rn(acc_var, __dmul_rn(sj, sj)); }
                 if (c.refined) c.refined[cell] = kept ? 1 : 0;
             }
@@ -524,11 +595,11 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
         }
         const double gm = zmc_block_sum(acc_mu, smem);
         const double gv = zmc_block_sum(acc_var, smem);
-        if (threadIdx.x == 0) { c.gacc[2 * G] = gm; c.gacc[2 * G + 1] = gv; }
+        if (threadIdx.x == 0) { c.gacc[2 * tile] = gm; c.gacc[2 * tile + 1] = gv; }
     }
 }
 
-/* R7: value_b += sum of accepted mu ; var_b += sum of accepted s^2, one block per instance */
+/* R7: value_b += sum of accepted mu ; var_b += sum of accepted s^2, one block per instance, over its tiles */
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_accumulate_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
     for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
