@@ -321,3 +321,118 @@ def run(cfg: Config, keep_cells: bool = False) -> Result:
         return Result(value, std, levels, L.orc_total_evals(h))
     finally:
         L.orc_free(h)
+
+
+# ------------------------------------------------------------------ R15: vector-valued user integrands (zmc_oracle_vec.cpp)
+USER_F64 = C.CFUNCTYPE(None, C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_double), C.c_int)
+USER_F32 = C.CFUNCTYPE(None, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_float), C.c_int)
+
+
+def compile_user_fn(src: str, fn_name: str, precisions=("f64", "f32")):
+    """Compile a user integrand -- the very text handed to zmc_set_integrand_source_vec, `__device__` defined away --
+    with g++ (-O2 -ffp-contract=off, like the oracle) and return (f64, f32) C function pointers (None where not asked
+    for). The user function is an input of the method, not part of it. The text must be plain C++ valid on both sides."""
+    import hashlib
+    import os
+    import subprocess
+    import tempfile
+    wrap = ["#include <math.h>\n#define __device__\n#define __forceinline__ inline\n", src, "\n"]
+    if "f64" in precisions:
+        wrap.append('extern "C" void orc_user_entry_f64(const double* x, int dim, const double* p, int np, double* out, int n_out) '
+                    "{ %s(x, dim, p, np, out, n_out); }\n" % fn_name)
+    if "f32" in precisions:
+        wrap.append('extern "C" void orc_user_entry_f32(const float* x, int dim, const float* p, int np, float* out, int n_out) '
+                    "{ %s(x, dim, p, np, out, n_out); }\n" % fn_name)
+    text = "".join(wrap)
+    d = os.path.join(tempfile.gettempdir(), "zmc_oracle_user")
+    os.makedirs(d, exist_ok=True)
+    tag = hashlib.sha256(text.encode()).hexdigest()[:24]
+    so = os.path.join(d, "user_%s.so" % tag)
+    if not os.path.exists(so):
+        cpp = os.path.join(d, "user_%s.cpp" % tag)
+        with open(cpp, "w") as f:
+            f.write(text)
+        tmp = so + ".tmp%d" % os.getpid()
+        subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-mfma", "-fPIC", "-shared", "-o", tmp, cpp], check=True)
+        os.replace(tmp, so)
+    L = C.CDLL(so)
+    f64 = C.cast(L.orc_user_entry_f64, USER_F64) if "f64" in precisions else None
+    f32 = C.cast(L.orc_user_entry_f32, USER_F32) if "f32" in precisions else None
+    return f64, f32
+
+
+def _vec_lib():
+    L = lib()
+    if not getattr(L, "_vec_ready", False):
+        u32p, u64p, dp = C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_double)
+        L.orc_vec_unit_sums.argtypes = [C.POINTER(_Cfg), C.c_int, USER_F64, USER_F32, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, dp]
+        L.orc_run_vec.argtypes = [C.POINTER(_Cfg), C.c_int, USER_F64, USER_F32, C.c_int]
+        L.orc_run_vec.restype = C.c_void_p
+        L.orc_vec_free.argtypes = [C.c_void_p]
+        L.orc_vec_error.argtypes = [C.c_void_p]
+        L.orc_vec_error.restype = C.c_char_p
+        L.orc_vec_get.argtypes = [C.c_void_p, dp, dp]
+        L.orc_vec_levels.argtypes = [C.c_void_p]
+        L.orc_vec_total_evals.argtypes = [C.c_void_p]
+        L.orc_vec_total_evals.restype = C.c_uint64
+        L.orc_vec_level_counts.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.orc_vec_level_cells.argtypes = [C.c_void_p, C.c_int, u32p, u64p, u32p, dp, dp, dp, C.POINTER(C.c_uint8), dp]
+        L.orc_vec_level_cells.restype = C.c_int64
+        L._vec_ready = True
+    return L
+
+
+def _fn_args(fns):
+    f64, f32 = fns
+    return (f64 if f64 is not None else C.cast(None, USER_F64)), (f32 if f32 is not None else C.cast(None, USER_F32))
+
+
+def vec_unit_sums(cfg: Config, n_components, fns, instance, path, level, coords, trial):
+    """R15: the n_components sums of one (cell, trial) unit. fns = compile_user_fn(...)."""
+    cc = np.ascontiguousarray(coords, dtype=np.uint32)
+    S = np.zeros(n_components)
+    c = cfg.c()
+    f64, f32 = _fn_args(fns)
+    rc = _vec_lib().orc_vec_unit_sums(C.byref(c), n_components, f64, f32, instance, path & (2**64 - 1), path >> 64, level,
+                                      _u32p(cc), trial, _dp(S))
+    if rc != 0:
+        raise ValueError("oracle: bad config")
+    return S
+
+
+def run_vec(cfg: Config, n_components, fns, keep_cells: bool = False) -> Result:
+    """R15: the whole tree of a vector-valued user integrand. value, std: [n_instances, n_components];
+    per level (keep_cells) mu, s, tau: [cells, C], S: [cells, T, C]."""
+    L = _vec_lib()
+    c = cfg.c()
+    f64, f32 = _fn_args(fns)
+    h = L.orc_run_vec(C.byref(c), n_components, f64, f32, 1 if keep_cells else 0)
+    try:
+        err = L.orc_vec_error(h)
+        if err:
+            raise ValueError("oracle: " + err.decode())
+        nc = n_components
+        value = np.zeros((cfg.n_instances, nc))
+        std = np.zeros((cfg.n_instances, nc))
+        L.orc_vec_get(h, _dp(value), _dp(std))
+        levels = []
+        for lev in range(1, L.orc_vec_levels(h) + 1):
+            a, b, t = C.c_int64(), C.c_int64(), C.c_int64()
+            L.orc_vec_level_counts(h, lev, C.byref(a), C.byref(b), C.byref(t))
+            rec = Level(a.value, b.value, t.value)
+            if keep_cells:
+                n = a.value
+                inst = np.zeros(n, dtype=np.uint32)
+                plo = np.zeros(n, dtype=np.uint64)
+                phi = np.zeros(n, dtype=np.uint32)
+                mu, s, tau = np.zeros((n, nc)), np.zeros((n, nc)), np.zeros((n, nc))
+                ref = np.zeros(n, dtype=np.uint8)
+                S = np.zeros((n, cfg.trials, nc))
+                L.orc_vec_level_cells(h, lev, _u32p(inst), plo.ctypes.data_as(C.POINTER(C.c_uint64)), _u32p(phi),
+                                      _dp(mu), _dp(s), _dp(tau), ref.ctypes.data_as(C.POINTER(C.c_uint8)), _dp(S))
+                rec.instance, rec.mu, rec.s, rec.tau, rec.refined, rec.S = inst, mu, s, tau, ref, S
+                rec.path = [int(phi[i]) << 64 | int(plo[i]) for i in range(n)]
+            levels.append(rec)
+        return Result(value, std, levels, L.orc_vec_total_evals(h))
+    finally:
+        L.orc_vec_free(h)

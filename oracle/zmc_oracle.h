@@ -16,7 +16,8 @@
  * standard deviations and how cell stds are "collected" are
  * readings, "parity unpinned" by the paper (its tables print no formula and
  * its numbers match none exactly); everything else is pinned in
- * tests/test_oracle_*.py.
+ * tests/test_oracle_*.py. The "any component" flag rule of vector-valued integrands
+ * (R15, zmc_oracle_vec.cpp) is a reading as well: parity unpinned by the paper.
  */
 #ifndef ZMC_ORACLE_H
 #define ZMC_ORACLE_H
@@ -110,6 +111,26 @@ int64_t orc_level_cells(const orc_result*, int level, uint32_t* instance, uint64
 
 /* R13: per-(cell, trial) sums of squares of one level, [cells*T]; 0 cells unless spread = samples and keep_cells */
 int64_t orc_level_sumsq(const orc_result*, int level, double* Q);
+
+/* ---- R15: vector-valued user integrands (zmc_oracle_vec.cpp). The user function is an input of the method: it writes
+ * n_out components of f at the point x (the FP64 or the FP32 arithmetic, by cfg->precision). cfg->integrand is ignored;
+ * group scope, breadth-first, spread from the trials, path-order budget only. ---- */
+typedef void (*orc_user_f64)(const double* x, int dim, const double* p, int np, double* out, int n_out);
+typedef void (*orc_user_f32)(const float* x, int dim, const float* p, int np, float* out, int n_out);
+typedef struct orc_vec_result orc_vec_result;
+/* S[j] = sum_s (double) f_j(x_s) of one (cell, trial) unit, j = 0 .. n_components-1 */
+int orc_vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
+                      uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S);
+orc_vec_result* orc_run_vec(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, int keep_cells);
+void orc_vec_free(orc_vec_result*);
+const char* orc_vec_error(const orc_vec_result*);
+void orc_vec_get(const orc_vec_result*, double* value, double* std);   /* [n_instances * n_components], component fastest */
+int orc_vec_levels(const orc_vec_result*);
+uint64_t orc_vec_total_evals(const orc_vec_result*);
+void orc_vec_level_counts(const orc_vec_result*, int level, int64_t* n_cells, int64_t* n_refined, int64_t* n_truncated);
+/* mu, s, tau: [cells * C]; S: [cells * T * C] (trial-major, component fastest); any pointer may be NULL */
+int64_t orc_vec_level_cells(const orc_vec_result*, int level, uint32_t* instance, uint64_t* path_lo, uint32_t* path_hi,
+                            double* mu, double* s, double* tau, uint8_t* refined, double* S);
 
 #ifdef __cplusplus
 }

@@ -1,5 +1,5 @@
 """the oracle built with -fsanitize=address,undefined runs the worked example (config 1) and a small
-batched FP32 tree with every option on (budget, R13 spread, R14 order, kept cells, DFS) without a report, and gives the
+batched FP32 tree with every option on (budget, R13 spread, R14 order, kept cells, DFS) and a vector-valued run (R15) without a report, and gives the
 golden value. A plain executable, not the ctypes library: ASan wants to be the first thing loaded in its process."""
 import os
 import subprocess
@@ -12,6 +12,9 @@ MAIN = r"""
 #include <cstdlib>
 #include <vector>
 #include "zmc_oracle.h"
+
+static void user2_f64(const double* x, int, const double* p, int, double* out, int) { out[0] = p[0] * x[0] * x[0]; out[1] = x[1]; }
+static void user2_f32(const float* x, int, const float* p, int, float* out, int) { out[0] = p[0] * x[0] * x[0]; out[1] = x[1]; }
 
 static int run(orc_config& c, int keep, double* value, double* std_) {
     orc_result* r = orc_run(&c, keep);
@@ -58,6 +61,29 @@ int main() {
     double bv[3], bs[3];
     if (run(b, 1, bv, bs)) return 1;
     std::printf("batched %.6f %.6f %.6f\n", bv[0], bv[1], bv[2]);
+    /* R15: a two-component user integrand in FP32, two instances, depth 3, budget 3, kept cells */
+    {
+        double pv[2][1] = {{1.0}, {2.0}};
+        orc_config v2c = {};
+        v2c.dim = 2; v2c.g = 4; v2c.trials = 3; v2c.depth = 3; v2c.n_samples = 77; v2c.seed = 4; v2c.sigma_multiplier = 0.5;
+        v2c.precision = ORC_F32; v2c.n_instances = 2; v2c.params_per_instance = 1;
+        v2c.lower = lo2; v2c.upper = up2; v2c.params = &pv[0][0]; v2c.max_groups_per_level = 3;
+        orc_vec_result* vr = orc_run_vec(&v2c, 2, user2_f64, user2_f32, 1);
+        if (!vr || orc_vec_error(vr)) { std::printf("vec error\n"); return 5; }
+        double vv[4], vs[4];
+        orc_vec_get(vr, vv, vs);
+        for (int l = 1; l <= orc_vec_levels(vr); ++l) {
+            int64_t n = 0;
+            orc_vec_level_counts(vr, l, &n, nullptr, nullptr);
+            std::vector<uint32_t> inst(n), phi(n);
+            std::vector<uint64_t> plo(n);
+            std::vector<double> mu(2 * n), s(2 * n), tau(2 * n), S(2 * n * v2c.trials);
+            std::vector<uint8_t> ref(n);
+            if (orc_vec_level_cells(vr, l, inst.data(), plo.data(), phi.data(), mu.data(), s.data(), tau.data(), ref.data(), S.data()) != n) return 6;
+        }
+        std::printf("vec %.6f %.6f %.6f %.6f\n", vv[0], vv[1], vv[2], vv[3]);
+        orc_vec_free(vr);
+    }
     /* a config the oracle must refuse cleanly */
     b.trials = 300;
     orc_result* r = orc_run(&b, 0);
@@ -74,7 +100,8 @@ def test_oracle_under_asan_ubsan():
         exe = os.path.join(d, "orc_san")
         cmd = ["g++", "-O1", "-g", "-std=c++17", "-ffp-contract=off", "-mfma", "-fsanitize=address,undefined",
                "-fno-sanitize-recover=all", "-fno-omit-frame-pointer", "-I", os.path.join(ROOT, "oracle"),
-               os.path.join(d, "main.cpp"), os.path.join(ROOT, "oracle", "zmc_oracle.cpp"), "-o", exe]
+               os.path.join(d, "main.cpp"), os.path.join(ROOT, "oracle", "zmc_oracle.cpp"),
+               os.path.join(ROOT, "oracle", "zmc_oracle_vec.cpp"), "-o", exe]
         subprocess.run(cmd, check=True)
         env = dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", UBSAN_OPTIONS="print_stacktrace=1")
         r = subprocess.run([exe], capture_output=True, text=True, env=env)
