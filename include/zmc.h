@@ -31,6 +31,7 @@ extern "C" {
 #define ZMC_MAX_DIM 16      /* D <= 16 (D <= 12 pre-compiled, 13..16 JIT-compiled) */
 #define ZMC_MAX_DEPTH 15    /* level fits 4 bits of the Philox counter (R3) */
 #define ZMC_MAX_TRIALS 255  /* trial fits 8 bits of the Philox counter (R3) */
+#define ZMC_MAX_COMPONENTS 16 /* components of a vector-valued user integrand (R15) */
 
 typedef enum zmc_status {
     ZMC_OK = 0,
@@ -41,7 +42,8 @@ typedef enum zmc_status {
     ZMC_ERR_CUDA = -5,         /* a CUDA runtime call failed (or no device) */
     ZMC_ERR_CAPACITY = -6,     /* a level needed more cells than max_cells_per_level; result invalid */
     ZMC_ERR_NOT_RUN = -7,      /* zmc_result / zmc_stats / zmc_level_cells before zmc_run */
-    ZMC_ERR_STATE = -8         /* option changed after the workspace was fixed, level stats not kept ... */
+    ZMC_ERR_STATE = -8         /* option changed after the workspace was fixed, level stats not kept, an option not defined for a
+                                  vector-valued integrand ... */
 } zmc_status;
 
 /* Built-in integrands. params = [n_instances][params_per_instance] doubles.
@@ -115,6 +117,19 @@ int zmc_set_integrand(zmc_ctx* ctx, int builtin_id, const double* params, int pa
 int zmc_set_integrand_source(zmc_ctx* ctx, const char* cuda_src, const char* fn_name, const double* params,
                              int params_per_instance, int n_instances);
 
+/* A VECTOR-VALUED user integrand (R15; the paper's "general user defined functions", and its application with
+ * an integrand of "several thousands terms"): n_components values f_0 .. f_{C-1} per point, 1 <= C <= ZMC_MAX_COMPONENTS,
+ * all evaluated at the same sample points -- one random stream and one map per (cell, trial) unit, C FP64 sums. cuda_src [host] must define
+ *     __device__ void fn_name(const float*  x, int dim, const float*  p, int np, float*  out, int n_out)   (ZMC_F32)
+ *     __device__ void fn_name(const double* x, int dim, const double* p, int np, double* out, int n_out)   (ZMC_F64)
+ * which writes out[0 .. n_out), n_out = n_components. Each component gets its own per-cell (mu, s) and per-group threshold; a cell is
+ * refined iff SOME component's s exceeds that component's threshold; zmc_result then returns n_instances * n_components values and
+ * stds, [instance][component], and the per-cell arrays of zmc_level_cells* carry C entries per cell (mu, s, tau: [cell*C + j];
+ * S: [(cell*T + t)*C + j]). Compiled during this call like zmc_set_integrand_source. ZMC_ERR_STATE if ZMC_SPREAD_SAMPLES is in force,
+ * or ZMC_BUDGET_LARGEST_SPREAD with C > 1 (not defined for several components); ZMC_ERR_RANGE for C outside 1..16. */
+int zmc_set_integrand_source_vec(zmc_ctx* ctx, const char* cuda_src, const char* fn_name, int n_components, const double* params,
+                                 int params_per_instance, int n_instances);
+
 /* Returns ZMC_ERR_ARG for an unknown key or a value out of range, ZMC_ERR_STATE for a value that changes the workspace
  * layout (KEEP_LEVEL_STATS, MAX_CELLS_PER_LEVEL, TARGET_ITEMS, SPREAD, BUDGET_ORDER) after zmc_set_workspace has fixed a
  * caller-owned workspace and a run has laid it out. On any error the context is unchanged. */
@@ -136,7 +151,8 @@ int zmc_run(zmc_ctx* ctx, void* cuda_stream);
 
 /* Synchronise the run's stream and fetch, per instance, the integral estimate (sum of accepted cell
  * means) and its standard deviation (sqrt of the sum of accepted cell variances, R7).
- * value, std [host] n_instances doubles each. Returns ZMC_ERR_CAPACITY if a level overflowed. */
+ * value, std [host] n_instances doubles each (n_instances * n_components, [instance][component], for a vector-valued
+ * integrand). Returns ZMC_ERR_CAPACITY if a level overflowed. */
 int zmc_result(zmc_ctx* ctx, double* value, double* std);
 
 typedef struct zmc_level_stats {
@@ -199,7 +215,8 @@ int zmc_debug_words(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t 
 
 /* Sample points and integrand values of the first n samples of one unit, produced by the same device
  * functions the sampling kernel uses. coords [host] D level-`level` integer cell coordinates.
- * x [host] n*D doubles (FP32 mode: floats widened; EXP_QUAD in FP32: x - c, R8), f [host] n doubles. */
+ * x [host] n*D doubles (FP32 mode: floats widened; EXP_QUAD in FP32: x - c, R8), f [host] n doubles
+ * (n * n_components, component fastest, for a vector-valued integrand). */
 int zmc_debug_points(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
                      const uint32_t* coords, int trial, uint64_t n, double* x, double* f);
 

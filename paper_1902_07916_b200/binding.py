@@ -30,7 +30,7 @@ F64, F32 = 0, 1
 MATH_EXACT, MATH_FAST = 0, 1
 MAX_DEPTH = 15
 
-EXPORTS = ["zmc_create", "zmc_set_integrand", "zmc_set_integrand_source", "zmc_set_option", "zmc_workspace_bytes",
+EXPORTS = ["zmc_create", "zmc_set_integrand", "zmc_set_integrand_source", "zmc_set_integrand_source_vec", "zmc_set_option", "zmc_workspace_bytes",
            "zmc_set_workspace", "zmc_run", "zmc_result", "zmc_stats", "zmc_level_cells", "zmc_level_cells_range", "zmc_level_sumsq", "zmc_debug_words",
            "zmc_debug_points", "zmc_last_error", "zmc_status_string", "zmc_destroy"]
 
@@ -79,6 +79,7 @@ def lib():
     L.zmc_create.argtypes = [C.POINTER(vp), C.c_int, dp, dp, C.c_int, C.c_uint64, C.c_int, C.c_int, C.c_double, C.c_uint64]
     L.zmc_set_integrand.argtypes = [vp, C.c_int, dp, C.c_int, C.c_int]
     L.zmc_set_integrand_source.argtypes = [vp, C.c_char_p, C.c_char_p, dp, C.c_int, C.c_int]
+    L.zmc_set_integrand_source_vec.argtypes = [vp, C.c_char_p, C.c_char_p, C.c_int, dp, C.c_int, C.c_int]
     L.zmc_set_option.argtypes = [vp, C.c_int, C.c_int64]
     L.zmc_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     L.zmc_set_workspace.argtypes = [vp, vp, C.c_size_t]
@@ -128,6 +129,7 @@ class Integrator:
         self._h = C.c_void_p()
         self.dim, self.trials, self.depth = dim, trials, depth
         self.n_instances = 1
+        self.n_components = 0       # 0: scalar integrand; C >= 1: vector-valued user integrand, results carry a component axis
         lo = np.ascontiguousarray(lower, dtype=np.float64)
         up = np.ascontiguousarray(upper, dtype=np.float64)
         rc = self._L.zmc_create(C.byref(self._h), dim, _dp(lo), _dp(up), divisions_per_axis, samples_per_cell,
@@ -166,6 +168,7 @@ class Integrator:
             ppi = p.shape[1]
         self._check(self._L.zmc_set_integrand(self._h, builtin_id, _dp(p), ppi, n_instances))
         self.n_instances = n_instances
+        self.n_components = 0
 
     def set_integrand_source(self, cuda_src: str, fn_name: str, params: Optional[np.ndarray] = None, n_instances: int = 1):
         if params is None:
@@ -175,6 +178,22 @@ class Integrator:
             ppi = p.shape[1]
         self._check(self._L.zmc_set_integrand_source(self._h, cuda_src.encode(), fn_name.encode(), _dp(p), ppi, n_instances))
         self.n_instances = n_instances
+        self.n_components = 0
+
+    def set_integrand_source_vec(self, cuda_src: str, fn_name: str, n_components: int, params: Optional[np.ndarray] = None,
+                                 n_instances: int = 1):
+        if params is None:
+            p, ppi = None, 0
+        else:
+            p = np.ascontiguousarray(params, dtype=np.float64).reshape(n_instances, -1)
+            ppi = p.shape[1]
+        self._check(self._L.zmc_set_integrand_source_vec(self._h, cuda_src.encode(), fn_name.encode(), n_components, _dp(p), ppi, n_instances))
+        self.n_instances = n_instances
+        self.n_components = n_components
+
+    def _cshape(self, *lead):
+        """Array shape of a per-`lead` quantity: a trailing component axis for vector-valued integrands."""
+        return tuple(lead) + ((self.n_components,) if self.n_components else ())
 
     def set_option(self, key: int, value: int):
         self._check(self._L.zmc_set_option(self._h, key, int(value)))
@@ -203,8 +222,8 @@ class Integrator:
         self._check(self._L.zmc_run(self._h, C.c_void_p(stream)))
 
     def result(self):
-        v = np.zeros(self.n_instances)
-        s = np.zeros(self.n_instances)
+        v = np.zeros(self._cshape(self.n_instances))
+        s = np.zeros(self._cshape(self.n_instances))
         self._check(self._L.zmc_result(self._h, _dp(v), _dp(s)))
         return v, s
 
@@ -220,9 +239,9 @@ class Integrator:
         inst = np.zeros(n, dtype=np.uint32)
         plo = np.zeros(n, dtype=np.uint64)
         phi = np.zeros(n, dtype=np.uint32)
-        mu, s, tau = np.zeros(n), np.zeros(n), np.zeros(n)
+        mu, s, tau = np.zeros(self._cshape(n)), np.zeros(self._cshape(n)), np.zeros(self._cshape(n))
         ref = np.zeros(n, dtype=np.uint8)
-        S = np.zeros((n, self.trials))
+        S = np.zeros(self._cshape(n, self.trials))
         nn = C.c_uint64()
         self._check(self._L.zmc_level_cells(self._h, level, n, C.byref(nn), _ptr(inst, C.c_uint32), _ptr(plo, C.c_uint64),
                                             _ptr(phi, C.c_uint32), _dp(mu), _dp(s), _dp(tau), _ptr(ref, C.c_uint8), _dp(S)))
@@ -233,9 +252,9 @@ class Integrator:
         inst = np.zeros(count, dtype=np.uint32)
         plo = np.zeros(count, dtype=np.uint64)
         phi = np.zeros(count, dtype=np.uint32)
-        mu, s, tau = np.zeros(count), np.zeros(count), np.zeros(count)
+        mu, s, tau = np.zeros(self._cshape(count)), np.zeros(self._cshape(count)), np.zeros(self._cshape(count))
         ref = np.zeros(count, dtype=np.uint8)
-        S = np.zeros((count, self.trials))
+        S = np.zeros(self._cshape(count, self.trials))
         self._check(self._L.zmc_level_cells_range(self._h, level, first, count, _ptr(inst, C.c_uint32), _ptr(plo, C.c_uint64),
                                                   _ptr(phi, C.c_uint32), _dp(mu), _dp(s), _dp(tau), _ptr(ref, C.c_uint8), _dp(S)))
         path = [(int(h) << 64) | int(l) for h, l in zip(phi, plo)]
@@ -255,7 +274,7 @@ class Integrator:
     def debug_points(self, instance: int, path: int, level: int, coords, trial: int, n: int):
         cc = np.ascontiguousarray(coords, dtype=np.uint32)
         x = np.zeros((n, self.dim))
-        f = np.zeros(n)
+        f = np.zeros(self._cshape(n))
         self._check(self._L.zmc_debug_points(self._h, instance, path & (2 ** 64 - 1), path >> 64, level,
                                              _ptr(cc, C.c_uint32), trial, n, _dp(x), _dp(f)))
         return x, f

@@ -41,6 +41,8 @@ struct ZmcCtlArgs {
     ZmcLevelInfo* info;     /* array indexed by level, 1..L+1 */
     zu32 level, L, T, g, D;
     zu32 n_inst;
+    zu32 nc;                /* components per cell (R15); 1 except for vector-valued user integrands. Per-cell arrays are
+                               [cell * nc + j], per-group ones [group * nc + j], per-tile ones [tile * nc + j], value/var [instance * nc + j] */
     zu64 k, N;
     zu32 sample_groups;     /* sample groups per unit = ceil(N / SG) */
     zu32 target_items, min_chunk_groups;
@@ -132,8 +134,7 @@ __global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) {
         c.cur.plo[b] = 0ull;
         c.cur.phi[b] = 0u;
         for (zu32 d = 0; d < c.D; ++d) c.cur.coord[(zu64)d * c.par_stride + b] = 0u;
-        c.value[b] = 0.0;
-        c.var[b] = 0.0;
+        for (zu32 j = 0; j < c.nc; ++j) { c.value[b * c.nc + j] = 0.0; c.var[b * c.nc + j] = 0.0; }
     }
     if (tid == 0) {
         for (zu32 l = 0; l <= c.L + 1; ++l) {
@@ -158,19 +159,23 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const _
     const zu32 nch = li.n_chunks;
     const double dN = (double)c.N, dT = (double)c.T;
     zu64 bad = 0;
-    for (zu64 cell = (zu64)blockIdx.x * blockDim.x + threadIdx.x; cell < n_cells; cell += (zu64)gridDim.x * blockDim.x) {
+    const zu64 nc = c.nc;
+    /* one thread per (cell, component): component j of work item i is partial[i * nc + j] (R15); nc == 1: one thread per cell */
+    for (zu64 e = (zu64)blockIdx.x * blockDim.x + threadIdx.x; e < n_cells * nc; e += (zu64)gridDim.x * blockDim.x) {
+        const zu64 cell = (nc == 1ull) ? e : e / nc;
+        const zu64 jc = e - cell * nc;
         double A = 1.0;
         if (c.prefactor_index >= 0) {
             const zu32 inst = c.cur.inst[cell / c.k];
             A = c.params[(zu64)inst * (zu64)c.ppi + (zu64)c.prefactor_index];
         }
         const double VA = __dmul_rn(c.V, A);
-        const double* p = c.partial + cell * (zu64)c.T * nch;
+        const double* p = c.partial + cell * (zu64)c.T * nch * nc + jc;
         double acc = 0.0;
         for (zu32 t = 0; t < c.T; ++t) {
-            double S = p[(zu64)t * nch];
-            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)t * nch + ch]);
-            if (c.S) c.S[cell * c.T + t] = S;
+            double S = p[(zu64)t * nch * nc];
+            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]);
+            if (c.S) c.S[(cell * c.T + t) * nc + jc] = S;
             acc = __dadd_rn(acc, __ddiv_rn(__dmul_rn(VA, S), dN));
         }
         const double mu = __ddiv_rn(acc, dT);
@@ -178,15 +183,15 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const _
         if (c.spread == 0) {
             double q = 0.0;
             for (zu32 t = 0; t < c.T; ++t) {
-                double S = p[(zu64)t * nch];
-                for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)t * nch + ch]);
+                double S = p[(zu64)t * nch * nc];
+                for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]);
                 const double d = __dadd_rn(__ddiv_rn(__dmul_rn(VA, S), dN), -mu);
                 q = __dadd_rn(q, __dmul_rn(d, d));
             }
             sd = __dsqrt_rn(__ddiv_rn(q, dT));
         } else {
             /* R13: Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples ; d = Qc - Sc^2/M, 0 unless d > Qc*2^-40 ;
-             * s = (V*A) * sqrt((d/M)/M), the standard error of mu */
+             * s = (V*A) * sqrt((d/M)/M), the standard error of mu. Scalar integrands only (nc == 1: the host refuses R13 otherwise) */
             const double* pq = c.partial_q + cell * (zu64)c.T * nch;
             double Sc = 0.0, Qc = 0.0;
             for (zu32 t = 0; t < c.T; ++t) {
@@ -201,8 +206,8 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const _
             if (!(d > __dmul_rn(Qc, 9.094947017729282e-13))) d = 0.0;
             sd = __dmul_rn(VA, __dsqrt_rn(__ddiv_rn(__ddiv_rn(d, M), M)));
         }
-        c.mu[cell] = mu;
-        c.s[cell] = sd;
+        c.mu[e] = mu;
+        c.s[e] = sd;
         if (!(fabs(mu) <= 1.7976931348623157e308) || !(fabs(sd) <= 1.7976931348623157e308)) ++bad;
     }
     if (bad) atomicAdd(c.nonfinite, bad);
@@ -251,25 +256,36 @@ struct ZmcTile {
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
     __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
     const zu64 n_groups = c.info[c.level].n_groups;
     const double dk = (double)c.k;
+    const zu64 nc = c.nc;
     for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
-        const double* s = c.s + G * c.k;
-        double part = 0.0;
-        for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) part = __dadd_rn(part, s[j]);
-        const double mean = __ddiv_rn(zmc_block_sum(part, smem), dk);
-        part = 0.0;
-        for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) {
-            const double d = __dadd_rn(s[j], -mean);
-            part = __dadd_rn(part, __dmul_rn(d, d));
+        const double* s = c.s + G * c.k * nc;
+        for (zu64 jc = 0; jc < nc; ++jc) {      /* R15: one threshold per component */
+            double part = 0.0;
+            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) part = __dadd_rn(part, s[j * nc + jc]);
+            const double mean = __ddiv_rn(zmc_block_sum(part, smem), dk);
+            part = 0.0;
+            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) {
+                const double d = __dadd_rn(s[j * nc + jc], -mean);
+                part = __dadd_rn(part, __dmul_rn(d, d));
+            }
+            const double pstd = __dsqrt_rn(__ddiv_rn(zmc_block_sum(part, smem), dk));
+            const double tau = __dadd_rn(mean, __dmul_rn(c.m, pstd));
+            if (threadIdx.x == 0) { c.tau[G * nc + jc] = tau; tau_sh[jc] = tau; }
         }
-        const double pstd = __dsqrt_rn(__ddiv_rn(zmc_block_sum(part, smem), dk));
-        const double tau = __dadd_rn(mean, __dmul_rn(c.m, pstd));
+        __syncthreads();
         zu64 n = 0;
         if (c.level < c.L)
-            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) n += (s[j] > tau) ? 1ull : 0ull;
+            for (zu64 j = threadIdx.x; j < c.k; j += ZMC_CTL_THREADS) {
+                bool any = false;       /* R15: flagged iff some component's spread passes its threshold */
+                for (zu64 jc = 0; jc < nc; ++jc) any = any || (s[j * nc + jc] > tau_sh[jc]);
+                n += any ? 1ull : 0ull;
+            }
         n = zmc_block_sum_u64(n, smem_u);
-        if (threadIdx.x == 0) { c.tau[G] = tau; c.cnt[G] = n; }
+        if (threadIdx.x == 0) c.cnt[G] = n;
+        __syncthreads();        /* tau_sh is rewritten by the next group */
     }
 }
 
@@ -278,9 +294,9 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __
  *   PASS 0  tsum[tile] = sum of s over the tile
  *   PASS 1  mean_G = (sum of the group's tsum, fixed shape) / k ;  tsq[tile] = sum of (s - mean_G)^2 over the tile
  *   PASS 2  pstd_G = sqrt((sum of the group's tsq) / k) ; tau_G = mean_G + m * pstd_G ; cnt[tile] = #(s > tau_G) in the tile */
-__device__ __forceinline__ double zmc_group_total(const double* t, zu64 G, zu32 tpg, double* smem) {
+__device__ __forceinline__ double zmc_group_total(const double* t, zu64 G, zu32 tpg, zu64 nc, zu64 jc, double* smem) {
     double part = 0.0;
-    for (zu32 i = threadIdx.x; i < tpg; i += ZMC_CTL_THREADS) part = __dadd_rn(part, t[G * tpg + i]);
+    for (zu32 i = threadIdx.x; i < tpg; i += ZMC_CTL_THREADS) part = __dadd_rn(part, t[(G * tpg + i) * nc + jc]);
     return zmc_block_sum(part, smem);
 }
 
@@ -288,30 +304,42 @@ template <int PASS>
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_pass_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
     __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
     const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
     const double dk = (double)c.k;
+    const zu64 nc = c.nc;
     for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const ZmcTile T(c, tile);
-        double mean = 0.0, tau = 0.0;
-        if (PASS >= 1) mean = __ddiv_rn(zmc_group_total(c.tsum, T.G, c.tpg, smem), dk);
-        if (PASS == 2) {
-            const double pstd = __dsqrt_rn(__ddiv_rn(zmc_group_total(c.tsq, T.G, c.tpg, smem), dk));
-            tau = __dadd_rn(mean, __dmul_rn(c.m, pstd));
-        }
-        double part = 0.0;
-        zu64 n = 0;
-        for (zu64 cell = T.c0 + threadIdx.x; cell < T.c1; cell += ZMC_CTL_THREADS) {
-            const double sj = c.s[cell];
-            if (PASS == 0) part = __dadd_rn(part, sj);
-            if (PASS == 1) { const double d = __dadd_rn(sj, -mean); part = __dadd_rn(part, __dmul_rn(d, d)); }
-            if (PASS == 2) n += (c.level < c.L && sj > tau) ? 1ull : 0ull;
-        }
-        if (PASS <= 1) {
+        for (zu64 jc = 0; jc < nc; ++jc) {      /* R15: per component */
+            double mean = 0.0;
+            if (PASS >= 1) mean = __ddiv_rn(zmc_group_total(c.tsum, T.G, c.tpg, nc, jc, smem), dk);
+            if (PASS == 2) {
+                const double pstd = __dsqrt_rn(__ddiv_rn(zmc_group_total(c.tsq, T.G, c.tpg, nc, jc, smem), dk));
+                const double tau = __dadd_rn(mean, __dmul_rn(c.m, pstd));
+                if (threadIdx.x == 0) { tau_sh[jc] = tau; if (tile == T.G * c.tpg) c.tau[T.G * nc + jc] = tau; }
+                continue;
+            }
+            double part = 0.0;
+            for (zu64 cell = T.c0 + threadIdx.x; cell < T.c1; cell += ZMC_CTL_THREADS) {
+                const double sj = c.s[cell * nc + jc];
+                if (PASS == 0) part = __dadd_rn(part, sj);
+                if (PASS == 1) { const double d = __dadd_rn(sj, -mean); part = __dadd_rn(part, __dmul_rn(d, d)); }
+            }
             const double tot = zmc_block_sum(part, smem);
-            if (threadIdx.x == 0) (PASS == 0 ? c.tsum : c.tsq)[tile] = tot;
-        } else {
+            if (threadIdx.x == 0) (PASS == 0 ? c.tsum : c.tsq)[tile * nc + jc] = tot;
+        }
+        if (PASS == 2) {
+            __syncthreads();
+            zu64 n = 0;
+            if (c.level < c.L)
+                for (zu64 cell = T.c0 + threadIdx.x; cell < T.c1; cell += ZMC_CTL_THREADS) {
+                    bool any = false;
+                    for (zu64 jc = 0; jc < nc; ++jc) any = any || (c.s[cell * nc + jc] > tau_sh[jc]);
+                    n += any ? 1ull : 0ull;
+                }
             n = zmc_block_sum_u64(n, smem_u);
-            if (threadIdx.x == 0) { c.cnt[tile] = n; if (tile == T.G * c.tpg) c.tau[T.G] = tau; }
+            if (threadIdx.x == 0) c.cnt[tile] = n;
+            __syncthreads();
         }
     }
 }
@@ -498,6 +526,9 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __gri
 /* R7: one block per tile. Flagged cells get their rank within the instance (stable, path
  * order); rank < B (R12) and slot < capacity -> the child record (R2) is written to the next parent
  * list. Every other cell is accepted: its mu and s^2 go into the tile's fixed-shape sums. */
+/* VEC (R15, nc > 1): a cell is flagged iff some component's spread passes that component's threshold, and the accepted sums are
+ * kept per component; the scalar instance is the code as it was. */
+template <bool VEC>
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
     __shared__ zu32 warp_cnt[ZMC_CTL_THREADS / 32], warp_cnt_eq[ZMC_CTL_THREADS / 32];
@@ -508,8 +539,9 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
         const ZmcTile T(c, tile);
         const zu64 G = T.G;
         const zu32 inst = c.cur.inst[G];
-        const double tau = c.tau[G];
-        const bool by_spread = (c.budget_order != 0) && (c.budget != ~0ull);
+        const zu64 nc = VEC ? (zu64)c.nc : 1ull;
+        const double tau = c.tau[G * nc];
+        const bool by_spread = !VEC && (c.budget_order != 0) && (c.budget != ~0ull);
         const zu64 gf = c.gfirst[inst];
         const zu64 r0 = c.excl[tile] - c.excl[gf];   /* flagged cells of this instance in earlier tiles */
         const zu64 r0_gt = by_spread ? c.excl_gt[tile] - c.excl_gt[gf] : 0ull;   /* ... above the pivot */
@@ -522,6 +554,9 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
         const zu64 j0 = T.c0 - G * c.k;              /* child index of the tile's first cell */
         const zu64 n_tile = T.c1 - T.c0;
         double acc_mu = 0.0, acc_var = 0.0;
+        double vacc_mu[VEC ? ZMC_DEV_MAX_COMPONENTS : 1], vacc_var[VEC ? ZMC_DEV_MAX_COMPONENTS : 1];
+        if constexpr (VEC)
+            for (int jc = 0; jc < ZMC_DEV_MAX_COMPONENTS; ++jc) { vacc_mu[jc] = 0.0; vacc_var[jc] = 0.0; }
         __syncthreads();
         if (threadIdx.x == 0) { run = 0; run_eq = 0; }
         __syncthreads();
@@ -532,9 +567,14 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
             double sj = 0.0, muj = 0.0;
             bool flag = false;
             if (i < n_tile) {
-                sj = c.s[cell];
-                muj = c.mu[cell];
-                flag = (c.level < c.L) && (sj > tau);
+                if constexpr (!VEC) {
+                    sj = c.s[cell];
+                    muj = c.mu[cell];
+                    flag = (c.level < c.L) && (sj > tau);
+                } else {
+                    for (zu64 jc = 0; jc < nc; ++jc) flag = flag || (c.s[cell * nc + jc] > c.tau[G * nc + jc]);
+                    flag = flag && (c.level < c.L);
+                }
             }
             /* path order: every flagged cell counts in `run`. Largest spread: cells above the pivot count in `run`,
              * cells at the pivot in `run_eq`; cells below it are not candidates. */
@@ -586,39 +626,57 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
                 }
             }
             if (i < n_tile) {
-                if (!kept) { acc_mu = __dadd_rn(acc_mu, muj); acc_var = __dadd_rn(acc_var, __dmul_rn(sj, sj)); }
+                if constexpr (!VEC) {
+                    if (!kept) { acc_mu = __dadd_rn(acc_mu, muj); acc_var = __dadd_rn(acc_var, __dmul_rn(sj, sj)); }
+                } else if (!kept) {
+                    for (zu64 jc = 0; jc < nc; ++jc) {
+                        const double sv = c.s[cell * nc + jc];
+                        vacc_mu[jc] = __dadd_rn(vacc_mu[jc], c.mu[cell * nc + jc]);
+                        vacc_var[jc] = __dadd_rn(vacc_var[jc], __dmul_rn(sv, sv));
+                    }
+                }
                 if (c.refined) c.refined[cell] = kept ? 1 : 0;
             }
             __syncthreads();
             if (threadIdx.x == 0) { run += tile_total; run_eq += tile_total_eq; }
             __syncthreads();
         }
-        const double gm = zmc_block_sum(acc_mu, smem);
-        const double gv = zmc_block_sum(acc_var, smem);
-        if (threadIdx.x == 0) { c.gacc[2 * tile] = gm; c.gacc[2 * tile + 1] = gv; }
+        if constexpr (!VEC) {
+            const double gm = zmc_block_sum(acc_mu, smem);
+            const double gv = zmc_block_sum(acc_var, smem);
+            if (threadIdx.x == 0) { c.gacc[2 * tile] = gm; c.gacc[2 * tile + 1] = gv; }
+        } else {
+            for (zu64 jc = 0; jc < nc; ++jc) {
+                const double gm = zmc_block_sum(vacc_mu[jc], smem);
+                const double gv = zmc_block_sum(vacc_var[jc], smem);
+                if (threadIdx.x == 0) { c.gacc[2 * (tile * nc + jc)] = gm; c.gacc[2 * (tile * nc + jc) + 1] = gv; }
+            }
+        }
     }
 }
 
 /* R7: value_b += sum of accepted mu ; var_b += sum of accepted s^2, one block per instance, over its tiles */
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_accumulate_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ double smem[ZMC_CTL_THREADS];
-    for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
+    const zu64 nc = c.nc;
+    for (zu64 e = blockIdx.x; e < (zu64)c.n_inst * nc; e += gridDim.x) {      /* one block per (instance, component) */
+        const zu64 b = e / nc, jc = e - b * nc;
         const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
         double am = 0.0, av = 0.0;
         for (zu64 G = g0 + threadIdx.x; G < g1; G += ZMC_CTL_THREADS) {
-            am = __dadd_rn(am, c.gacc[2 * G]);
-            av = __dadd_rn(av, c.gacc[2 * G + 1]);
+            am = __dadd_rn(am, c.gacc[2 * (G * nc + jc)]);
+            av = __dadd_rn(av, c.gacc[2 * (G * nc + jc) + 1]);
         }
         const double sm = zmc_block_sum(am, smem);
         const double sv = zmc_block_sum(av, smem);
         if (threadIdx.x == 0 && g1 > g0) {
-            c.value[b] = __dadd_rn(c.value[b], sm);
-            c.var[b] = __dadd_rn(c.var[b], sv);
+            c.value[e] = __dadd_rn(c.value[e], sm);
+            c.var[e] = __dadd_rn(c.var[e], sv);
         }
     }
 }
 
-/* result[b] = value_b ; result[n_inst + b] = sqrt(var_b) */
+/* result[b] = value_b ; result[n_inst + b] = sqrt(var_b)   (n_inst here = instances * components, R15) */
 __global__ void zmc_finalize_kernel(const double* value, const double* var, double* result, zu32 n_inst) {
     for (zu64 b = (zu64)blockIdx.x * blockDim.x + threadIdx.x; b < n_inst; b += (zu64)gridDim.x * blockDim.x) {
         result[b] = value[b];

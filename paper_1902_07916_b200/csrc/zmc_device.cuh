@@ -353,10 +353,25 @@ struct ZmcMapF64 {
  *   setup(args, instance, coords)  once per work item: geometry and this instance's parameters
  *   eval(words, xout)              one sample from D consecutive words -> the FP64 value the unit sum adds
  *                                  (xout != nullptr only in the debug kernel). */
+/* ZMC_USER_NC (R15): 0 = the user function returns its one value; n >= 1 = it is vector-valued and writes n components
+ * f_0 .. f_{n-1} of the same point: one word stream, one map, n FP64 sums per (cell, trial) unit. */
+#ifndef ZMC_USER_NC
+#define ZMC_USER_NC 0
+#endif
+#define ZMC_DEV_MAX_COMPONENTS 16
 #ifdef ZMC_USER_FN
+#if ZMC_USER_NC > 0
+__device__ void ZMC_USER_FN(const float* x, int dim, const float* p, int np, float* out, int n_out);
+__device__ void ZMC_USER_FN(const double* x, int dim, const double* p, int np, double* out, int n_out);
+#else
 __device__ float ZMC_USER_FN(const float* x, int dim, const float* p, int np);
 __device__ double ZMC_USER_FN(const double* x, int dim, const double* p, int np);
 #endif
+#endif
+template <int ID> struct ZmcComponents {
+    static constexpr bool VEC = (ID == ZMC_ID_USER) && (ZMC_USER_NC > 0);
+    static constexpr int NC = VEC ? ZMC_USER_NC : 1;
+};
 
 template <int ID, int D_, int PREC, int MODE>
 struct ZmcIntegrand;
@@ -365,6 +380,8 @@ template <int ID, int D_, int MODE>
 struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
     static constexpr int D = D_;
     static constexpr int PREC = ZMC_PREC_F32;
+    static constexpr bool VEC = ZmcComponents<ID>::VEC;
+    static constexpr int NC = ZmcComponents<ID>::NC;
     ZmcMapF32<D_> map;
     float c0;           /* CONST/LINEAR: p[0] ; EXP_QUAD: -a */
     float lin[ID == ZMC_ID_LINEAR ? D_ : 1];
@@ -438,10 +455,29 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F32, MODE> {
             if (MODE == ZMC_MODE_FAST) return zmc_fexp_value<CHK>(e);
             return zmc_zexp_value<CHK>(e);
         }
-#ifdef ZMC_USER_FN
+#if defined(ZMC_USER_FN) && ZMC_USER_NC == 0
         if (ID == ZMC_ID_USER) return (double)ZMC_USER_FN((const float*)x, D_, up, unp);
 #endif
         return 0.0;
+    }
+
+    /* R15: the NC components of a vector-valued user integrand at one sample point */
+    __device__ __forceinline__ void evalv(const zu32* w, double* out, double* xout) const {
+        float x[D_];
+#pragma unroll
+        for (int d = 0; d < D_; ++d) x[d] = map.x(d, w[d]);
+        if (xout) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) xout[d] = (double)x[d];
+        }
+#if defined(ZMC_USER_FN) && ZMC_USER_NC > 0
+        float o[NC];
+        ZMC_USER_FN((const float*)x, D_, up, unp, o, NC);
+#pragma unroll
+        for (int j = 0; j < NC; ++j) out[j] = (double)o[j];
+#else
+        out[0] = eval(w, nullptr);
+#endif
     }
 
     /* Two samples at once on the packed FP32 instructions: component-wise the operation sequence of eval(),
@@ -498,6 +534,8 @@ template <int ID, int D_, int MODE>
 struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
     static constexpr int D = D_;
     static constexpr int PREC = ZMC_PREC_F64;
+    static constexpr bool VEC = ZmcComponents<ID>::VEC;
+    static constexpr int NC = ZmcComponents<ID>::NC;
     ZmcMapF64<D_> map;
     double c0;          /* CONST/LINEAR: p[0] ; EXP_QUAD: a */
     double aux[(ID == ZMC_ID_LINEAR || ID == ZMC_ID_EXP_QUAD) ? D_ : 1];   /* LINEAR: coefficients ; EXP_QUAD: centre */
@@ -557,10 +595,24 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
             }
             return exp(-__dmul_rn(c0, q));
         }
-#ifdef ZMC_USER_FN
+#if defined(ZMC_USER_FN) && ZMC_USER_NC == 0
         if (ID == ZMC_ID_USER) return ZMC_USER_FN((const double*)x, D_, up, unp);
 #endif
         return 0.0;
+    }
+    __device__ __forceinline__ void evalv(const zu32* w, double* out, double* xout) const {
+        double x[D_];
+#pragma unroll
+        for (int d = 0; d < D_; ++d) x[d] = map.x(d, w[d]);
+        if (xout) {
+#pragma unroll
+            for (int d = 0; d < D_; ++d) xout[d] = x[d];
+        }
+#if defined(ZMC_USER_FN) && ZMC_USER_NC > 0
+        ZMC_USER_FN((const double*)x, D_, up, unp, out, NC);
+#else
+        out[0] = eval(w, nullptr);
+#endif
     }
     static constexpr bool HAS_PACKED = false;   /* there is no packed FP64 */
     template <bool CHK = true>
@@ -784,12 +836,58 @@ __device__ __forceinline__ void zmc_full_groups(const F& f, const ZmcKeySchedule
     if (gi < gfe) zmc_group_eval<F, SQ, CHK>(f, ks, uc, gi, acc, accq);
 }
 
+/* R15: one unit of a vector-valued integrand -- the same word stream and the same points as a scalar unit, NC FP64 sums,
+ * stored component-fastest at partial[out * NC + j]. One accumulator per component and lane (the user function, not the
+ * generator, sets the pace here), plain Philox calls. */
+template <class F>
+__device__ __forceinline__ void zmc_unit_vec(const ZmcSampleArgs& a, const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc,
+                                             zu32 lane, zu32 gb, zu32 ge, zu32 gfe, zu32 full_groups, zu32 tail, zu64 out) {
+    constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG, NC = F::NC;
+    double acc[NC];
+#pragma unroll
+    for (int j = 0; j < NC; ++j) acc[j] = 0.0;
+    for (zu32 gi = gb + lane; gi < gfe; gi += 32u) {
+        zu32 w[4 * CG];
+#pragma unroll
+        for (int c = 0; c < CG; ++c) zmc_philox(gi * (zu32)CG + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+#pragma unroll
+        for (int s = 0; s < SG; ++s) {
+            double o[NC];
+            f.evalv(&w[s * D], o, nullptr);
+#pragma unroll
+            for (int j = 0; j < NC; ++j) acc[j] = __dadd_rn(acc[j], o[j]);
+        }
+    }
+    if (tail != 0u && ge > full_groups && lane == 0u) {
+        zu32 w[4 * CG];
+        const zu32 q0 = full_groups * (zu32)CG;
+#pragma unroll
+        for (int c = 0; c < CG; ++c) zmc_philox(q0 + (zu32)c, uc.c1, uc.c2, uc.c3, ks, &w[4 * c]);
+#pragma unroll
+        for (int s = 0; s < SG; ++s)
+            if ((zu32)s < tail) {
+                double o[NC];
+                f.evalv(&w[s * D], o, nullptr);
+#pragma unroll
+                for (int j = 0; j < NC; ++j) acc[j] = __dadd_rn(acc[j], o[j]);
+            }
+    }
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+        double sum = acc[j];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
+        if (lane == 0u) a.partial[out * (zu64)NC + (zu64)j] = sum;
+    }
+}
+
 /* One (cell, trial, chunk) unit: the warp's lanes stride over the chunk's sample groups [gb, ge), lane 0 takes the ragged tail,
  * a shuffle reduction, one 8-byte store (two with SQ). */
 template <class F, bool SQ>
 __device__ __forceinline__ void zmc_unit(const ZmcSampleArgs& a, const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc,
                                          zu32 lane, zu32 gb, zu32 ge, zu32 gfe, zu32 full_groups, zu32 tail, zu64 out) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
+    if constexpr (F::VEC) { zmc_unit_vec<F>(a, f, ks, uc, lane, gb, ge, gfe, full_groups, tail, out); return; }
     /* acc[0..SG) sums the groups at even multiples of 32 from the lane's first one, acc[SG..2SG) those at odd multiples --
      * whatever UNROLL is, so results do not depend on it */
     double acc[2 * SG], accq[4];     /* sums of squares: two accumulators per group in flight are enough */
@@ -892,7 +990,7 @@ struct ZmcPointsArgs {
     zu32 coords[ZMC_DEV_MAX_DIM];
     zu64 n;
     double* x;              /* [n*D] */
-    double* f;              /* [n] */
+    double* f;              /* [n], vector-valued integrands: [n * NC], component fastest */
 };
 
 template <int D>
@@ -929,11 +1027,24 @@ __global__ void zmc_points_kernel(const __grid_constant__ ZmcPointsArgs pa) {
         zmc_sample_words<D>(s0, ks, uc, w0);
         zmc_sample_words<D>(s1, ks, uc, w1);
         double x0[D], x1[D];
+        if constexpr (F::VEC) {
+            double o0[F::NC], o1[F::NC];
+            f.evalv(w0, o0, x0);
+            f.evalv(w1, o1, x1);
+            if (pa.f) {
+#pragma unroll
+                for (int j = 0; j < F::NC; ++j) {
+                    pa.f[s0 * F::NC + j] = o0[j];
+                    if (s1 < pa.n) pa.f[s1 * F::NC + j] = o1[j];
+                }
+            }
+        } else {
         double v0 = f.eval(w0, x0), v1 = f.eval(w1, x1);
         if ((t & 1ull) == 0ull) f.eval2(w0, w1, v0, v1);
         if (pa.f) {
             pa.f[s0] = v0;
             if (s1 < pa.n) pa.f[s1] = v1;
+        }
         }
         if (pa.x) {
 #pragma unroll
