@@ -73,8 +73,14 @@ enum {
     ZMC_OPT_SPREAD = 9,               /* ZMC_SPREAD_TRIALS (default, the paper: s = std of the T trial estimates) or
                                          ZMC_SPREAD_SAMPLES (R13: s = standard error of the cell mean from sum f and
                                          sum f^2 of its T*N samples; zmc_result's std is then a 1-sigma error) */
-    ZMC_OPT_BUDGET_ORDER = 10         /* which flagged cells the budget keeps: ZMC_BUDGET_PATH_ORDER (default, R12) or
+    ZMC_OPT_BUDGET_ORDER = 10,        /* which flagged cells the budget keeps: ZMC_BUDGET_PATH_ORDER (default, R12) or
                                          ZMC_BUDGET_LARGEST_SPREAD (R14: the B largest s, equal ones in path order) */
+    ZMC_OPT_SINGLE_LAUNCH = 11        /* the whole tree search as ONE cooperative kernel launch (grid-wide barriers between the
+                                         sampling and control phases of every level) instead of 2 + 6*depth launches: for
+                                         launch-bound problems (BASELINE.json configs[0]; PAPER.md:162-184 is about this per-call
+                                         overhead). Same device functions, bit-identical results. 0 never, 1 whenever the kernel
+                                         exists (pre-compiled integrands, ZMC_SPREAD_TRIALS, path-order budget), 2 = auto (default):
+                                         when level 1 has at most 1e8 evaluations. zmc_stats: kernel_launches 1, per-level times 0 */
 };
 enum { ZMC_F64 = 0, ZMC_F32 = 1 };
 enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };
@@ -175,7 +181,8 @@ typedef struct zmc_stats_t {
     int32_t grid_blocks, block_threads;
     int32_t kernel_origin;          /* sampling kernel: 0 pre-compiled, 1 compiled by NVRTC for this context, 2 from the process-wide
                                        cache, 3 from the on-disk cache (ZMC_CACHE_DIR) */
-    int32_t kernel_launches;        /* kernels the last zmc_run enqueued (all the library's own; a CUDA graph replays the same nodes) */
+    int32_t kernel_launches;        /* kernels the last zmc_run enqueued (all the library's own; a CUDA graph replays the same nodes;
+                                       1 = the single-launch path, ZMC_OPT_SINGLE_LAUNCH) */
     zmc_level_stats level[ZMC_MAX_DEPTH];
 } zmc_stats_t;
 

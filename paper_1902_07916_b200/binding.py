@@ -23,7 +23,7 @@ OK, ERR_ARG, ERR_RANGE, ERR_NO_INTEGRAND, ERR_COMPILE, ERR_CUDA, ERR_CAPACITY, E
 CONST, LINEAR, SIN_SUM, EXP_QUAD, USER = 0, 1, 2, 3, 100
 OPT_PRECISION, OPT_MATH, OPT_MAX_GROUPS_PER_LEVEL, OPT_KEEP_LEVEL_STATS = 1, 2, 3, 4
 OPT_MAX_CELLS_PER_LEVEL, OPT_GRID_BLOCKS, OPT_TARGET_ITEMS, OPT_USE_GRAPH = 5, 6, 7, 8
-OPT_SPREAD, OPT_BUDGET_ORDER = 9, 10
+OPT_SPREAD, OPT_BUDGET_ORDER, OPT_SINGLE_LAUNCH = 9, 10, 11
 SPREAD_TRIALS, SPREAD_SAMPLES = 0, 1
 BUDGET_PATH_ORDER, BUDGET_LARGEST_SPREAD = 0, 1
 F64, F32 = 0, 1
@@ -282,7 +282,7 @@ class Integrator:
 
 def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool = False,
                   max_cells_per_level: int = 0, use_graph: bool = False, spread: int = SPREAD_TRIALS,
-                  budget_order: int = BUDGET_PATH_ORDER) -> Integrator:
+                  budget_order: int = BUDGET_PATH_ORDER, single_launch: Optional[int] = None) -> Integrator:
     """zmc_create + zmc_set_integrand + options for one of the seeded workloads."""
     it = Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
     it.set_integrand(_INTEGRAND_ID[w.integrand], w.params, w.n_instances)
@@ -294,6 +294,8 @@ def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool 
         it.set_option(OPT_KEEP_LEVEL_STATS, 1)
     if use_graph:
         it.set_option(OPT_USE_GRAPH, 1)
+    if single_launch is not None:
+        it.set_option(OPT_SINGLE_LAUNCH, single_launch)
     if spread != SPREAD_TRIALS:
         it.set_option(OPT_SPREAD, spread)
     if budget_order != BUDGET_PATH_ORDER:

@@ -20,6 +20,8 @@
  */
 #ifndef ZMC_CONTROL_CUH
 #define ZMC_CONTROL_CUH
+/* ZMC_CONTROL_BODIES_ONLY: the device functions (zmc_*_body) without the __global__ kernels around them -- for the translation
+ * units that only build the single-launch tree kernel (zmc_inst.cu); the kernels themselves are defined once, in zmc_lib.cu. */
 #include "zmc_device.cuh"
 
 #define ZMC_CTL_THREADS 256
@@ -115,6 +117,7 @@ __device__ __forceinline__ void zmc_plan_level(ZmcLevelInfo& li, zu64 n_groups, 
 }
 
 /* R3: Kd(seed, b) = words 0,1 of Philox(ctr = (b, 0, 0, 0x5A4D4321), key = (seed_lo, seed_hi)) */
+#ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void zmc_keys_kernel(zu32* keys, zu32 n_inst, zu32 seed_lo, zu32 seed_hi) {
     for (zu64 b = (zu64)blockIdx.x * blockDim.x + threadIdx.x; b < n_inst; b += (zu64)gridDim.x * blockDim.x) {
         ZmcKeySchedule ks;
@@ -125,11 +128,12 @@ __global__ void zmc_keys_kernel(zu32* keys, zu32 n_inst, zu32 seed_lo, zu32 seed
         keys[2 * b + 1] = w[1];
     }
 }
+#endif
 
 /* root parents (path 0, coordinates 0), zeroed results, the level-1 plan */
-__global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) {
-    const zu64 tid = (zu64)blockIdx.x * blockDim.x + threadIdx.x;
-    for (zu64 b = tid; b < c.n_inst; b += (zu64)gridDim.x * blockDim.x) {
+__device__ __forceinline__ void zmc_init_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
+    const zu64 tid = (zu64)bid * blockDim.x + threadIdx.x;
+    for (zu64 b = tid; b < c.n_inst; b += (zu64)nb * blockDim.x) {
         c.cur.inst[b] = (zu32)b;
         c.cur.plo[b] = 0ull;
         c.cur.phi[b] = 0u;
@@ -150,18 +154,21 @@ __global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) {
         *c.overflow = 0u;
     }
 }
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_init_kernel_body(c, blockIdx.x, gridDim.x); }
+#endif
 
 /* R5: S_t = sum of the chunk partials in chunk order ; I_t = ((V*A)*S_t)/(double)N ;
  * mu = (sum_t I_t)/T ; s = sqrt((sum_t (I_t-mu)^2)/T)  -- two-pass, population form. */
-__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const __grid_constant__ ZmcCtlArgs c) {
+/* the (cell, component) entries first, first + step, .. < last: one thread per entry */
+__device__ __forceinline__ void zmc_cell_stats_span(const ZmcCtlArgs& c, const zu64 first, const zu64 last, const zu64 step) {
     const ZmcLevelInfo& li = c.info[c.level];
-    const zu64 n_cells = li.n_cells;
     const zu32 nch = li.n_chunks;
     const double dN = (double)c.N, dT = (double)c.T;
     zu64 bad = 0;
     const zu64 nc = c.nc;
     /* one thread per (cell, component): component j of work item i is partial[i * nc + j] (R15); nc == 1: one thread per cell */
-    for (zu64 e = (zu64)blockIdx.x * blockDim.x + threadIdx.x; e < n_cells * nc; e += (zu64)gridDim.x * blockDim.x) {
+    for (zu64 e = first; e < last; e += step) {
         const zu64 cell = (nc == 1ull) ? e : e / nc;
         const zu64 jc = e - cell * nc;
         double A = 1.0;
@@ -212,6 +219,12 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const _
     }
     if (bad) atomicAdd(c.nonfinite, bad);
 }
+__device__ __forceinline__ void zmc_cell_stats_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
+    zmc_cell_stats_span(c, (zu64)bid * blockDim.x + threadIdx.x, c.info[c.level].n_cells * (zu64)c.nc, (zu64)nb * blockDim.x);
+}
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_cell_stats_kernel_body(c, blockIdx.x, gridDim.x); }
+#endif
 
 /* fixed-shape block reduction (sum); every thread gets the result */
 __device__ __forceinline__ double zmc_block_sum(double v, double* smem) {
@@ -253,14 +266,11 @@ struct ZmcTile {
 /* R6: one block per sibling group of at most ZMC_TILE_CELLS cells (tpg == 1); tau = mean(s) + m * pstd(s), both moments
  * two-pass, population form ("the mean and standard deviation of the calculated k standard deviations").
  * R7: flagged iff level < L and s > tau (strict; NaN compares false). */
-__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __grid_constant__ ZmcCtlArgs c) {
-    __shared__ double smem[ZMC_CTL_THREADS];
-    __shared__ zu64 smem_u[ZMC_CTL_THREADS];
-    __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
-    const zu64 n_groups = c.info[c.level].n_groups;
+/* one sibling group, by one block */
+__device__ __forceinline__ void zmc_threshold_group(const ZmcCtlArgs& c, const zu64 G, double* smem, zu64* smem_u, double* tau_sh) {
     const double dk = (double)c.k;
     const zu64 nc = c.nc;
-    for (zu64 G = blockIdx.x; G < n_groups; G += gridDim.x) {
+    {
         const double* s = c.s + G * c.k * nc;
         for (zu64 jc = 0; jc < nc; ++jc) {      /* R15: one threshold per component */
             double part = 0.0;
@@ -288,6 +298,44 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __
         __syncthreads();        /* tau_sh is rewritten by the next group */
     }
 }
+__device__ __forceinline__ void zmc_threshold_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
+    __shared__ double smem[ZMC_CTL_THREADS];
+    __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
+    const zu64 n_groups = c.info[c.level].n_groups;
+    for (zu64 G = bid; G < n_groups; G += nb) zmc_threshold_group(c, G, smem, smem_u, tau_sh);
+}
+
+/* Single-launch path, groups of one tile (tpg == 1), scalar integrands: one block takes a sibling group through its cell statistics
+ * (R5) AND its threshold and flag count (R6, R7) -- the block reads back only what it wrote itself, so a __syncthreads stands where
+ * the multi-launch path has a kernel boundary. On the last level (nothing can be flagged, R7) the group's accepted sums follow at
+ * once, in the shape zmc_scatter_kernel gives them, and the compaction step is skipped. Same arithmetic, same shapes, same bits. */
+__device__ __forceinline__ void zmc_group_control_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
+    __shared__ double smem[ZMC_CTL_THREADS];
+    __shared__ zu64 smem_u[ZMC_CTL_THREADS];
+    __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
+    const zu64 n_groups = c.info[c.level].n_groups;
+    for (zu64 G = bid; G < n_groups; G += nb) {
+        zmc_cell_stats_span(c, G * c.k + threadIdx.x, (G + 1ull) * c.k, blockDim.x);
+        __syncthreads();
+        zmc_threshold_group(c, G, smem, smem_u, tau_sh);
+        if (c.level >= c.L) {
+            double acc_mu = 0.0, acc_var = 0.0;
+            for (zu64 cell = G * c.k + threadIdx.x; cell < (G + 1ull) * c.k; cell += ZMC_CTL_THREADS) {
+                const double sj = c.s[cell];
+                acc_mu = __dadd_rn(acc_mu, c.mu[cell]);
+                acc_var = __dadd_rn(acc_var, __dmul_rn(sj, sj));
+                if (c.refined) c.refined[cell] = 0;
+            }
+            const double gm = zmc_block_sum(acc_mu, smem);
+            const double gv = zmc_block_sum(acc_var, smem);
+            if (threadIdx.x == 0) { c.gacc[2 * G] = gm; c.gacc[2 * G + 1] = gv; }
+        }
+    }
+}
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_threshold_kernel_body(c, blockIdx.x, gridDim.x); }
+#endif
 
 /* R6 for groups of more than ZMC_TILE_CELLS cells (tpg > 1): the same two-pass moments, one block per TILE and one launch per
  * pass, because each pass needs the whole group's previous one:
@@ -301,14 +349,14 @@ __device__ __forceinline__ double zmc_group_total(const double* t, zu64 G, zu32 
 }
 
 template <int PASS>
-__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_pass_kernel(const __grid_constant__ ZmcCtlArgs c) {
+__device__ __forceinline__ void zmc_threshold_pass_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
     __shared__ double smem[ZMC_CTL_THREADS];
     __shared__ zu64 smem_u[ZMC_CTL_THREADS];
     __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
     const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
     const double dk = (double)c.k;
     const zu64 nc = c.nc;
-    for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    for (zu64 tile = bid; tile < n_tiles; tile += nb) {
         const ZmcTile T(c, tile);
         for (zu64 jc = 0; jc < nc; ++jc) {      /* R15: per component */
             double mean = 0.0;
@@ -343,8 +391,10 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_pass_kernel(con
         }
     }
 }
+template <int PASS>
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_threshold_pass_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_threshold_pass_kernel_body<PASS>(c, blockIdx.x, gridDim.x); }
 
-/* block-wide exclusive scan of one value per thread (ZMC_SCAN_THREADS threads); returns the
+/* block-wide exclusive scan of one value per thread (any block of whole warps, up to 1024 threads); returns the
  * exclusive prefix and writes the block total to *total */
 __device__ __forceinline__ zu64 zmc_scan_block_excl(zu64 v, zu64* warp_tot, zu64* total) {
     const zu32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -358,7 +408,7 @@ __device__ __forceinline__ zu64 zmc_scan_block_excl(zu64 v, zu64* warp_tot, zu64
     if (lane == 31u) warp_tot[warp] = inc;
     __syncthreads();
     if (warp == 0) {
-        zu64 w = warp_tot[lane];
+        zu64 w = (lane < (blockDim.x >> 5)) ? warp_tot[lane] : 0ull;
         zu64 winc = w;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
@@ -375,15 +425,16 @@ __device__ __forceinline__ zu64 zmc_scan_block_excl(zu64 v, zu64* warp_tot, zu64
 /* One block. (A) exclusive scan of cnt over the tiles and the first/last tile of every instance
  * (groups, hence tiles, are sorted by instance); (B) per instance: flagged c_b, kept = min(c_b, B) (R12), exclusive
  * scan -> first output slot; (C) the next level's plan. */
-__global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid_constant__ ZmcCtlArgs c) {
+__device__ __forceinline__ void zmc_scan_kernel_body(const ZmcCtlArgs& c) {
+    const zu32 NT = blockDim.x;     /* ZMC_SCAN_THREADS as its own launch; the block size of the single-launch tree kernel inside it */
     __shared__ zu64 warp_tot[32];
     __shared__ zu64 total;
     __shared__ zu64 carry;
     const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
-    for (zu64 b = threadIdx.x; b < c.n_inst; b += ZMC_SCAN_THREADS) { c.gfirst[b] = 0; c.gend[b] = 0; }
+    for (zu64 b = threadIdx.x; b < c.n_inst; b += NT) { c.gfirst[b] = 0; c.gend[b] = 0; }
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
-    for (zu64 base = 0; base < n_tiles; base += ZMC_SCAN_THREADS) {
+    for (zu64 base = 0; base < n_tiles; base += NT) {
         const zu64 t = base + threadIdx.x;
         const zu64 v = (t < n_tiles) ? c.cnt[t] : 0ull;
         const zu64 ex = zmc_scan_block_excl(v, warp_tot, &total);
@@ -401,7 +452,7 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid
     __syncthreads();
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
-    for (zu64 base = 0; base < c.n_inst; base += ZMC_SCAN_THREADS) {
+    for (zu64 base = 0; base < c.n_inst; base += NT) {
         const zu64 b = base + threadIdx.x;
         zu64 kept = 0;
         if (b < c.n_inst) {
@@ -427,11 +478,15 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid
         c.info[c.level + 1] = li;
     }
 }
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_scan_kernel_body(c); }
+#endif
 
 /* ------------------------------------------------------------------ R14: the budget keeps the largest spreads */
 /* One block per instance: if more than B cells are flagged, radix-select (8 passes of 8 bits over the bit pattern
  * of s, which orders positive doubles) the B-th largest flagged spread -> piv, and how many cells equal to it are
  * kept -> quota = B - #(s > pivot). Otherwise piv = 0 and quota = all: no flagged cell is dropped (s >= +0, i.e. key >= 0). */
+#ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu32 hist[256];
     __shared__ zu64 sh_prefix, sh_need, sh_above;
@@ -474,8 +529,10 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __gr
         if (threadIdx.x == 0) { c.piv[b] = sh_prefix; c.quota[b] = c.budget - sh_above; }
     }
 }
+#endif
 
 /* per tile: flagged cells above and at the instance's pivot */
+#ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_count2_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu64 smem_u[ZMC_CTL_THREADS];
     const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
@@ -498,8 +555,10 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_count2_kernel(const __gri
         if (threadIdx.x == 0) { c.cnt_gt[tile] = ngt; c.cnt_eq[tile] = neq; }
     }
 }
+#endif
 
 /* One block: exclusive scans of cnt_gt and cnt_eq over the tiles. */
+#ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __grid_constant__ ZmcCtlArgs c) {
     __shared__ zu64 warp_tot[32];
     __shared__ zu64 total;
@@ -522,6 +581,7 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __gri
         }
     }
 }
+#endif
 
 /* R7: one block per tile. Flagged cells get their rank within the instance (stable, path
  * order); rank < B (R12) and slot < capacity -> the child record (R2) is written to the next parent
@@ -529,13 +589,13 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_scan2_kernel(const __gri
 /* VEC (R15, nc > 1): a cell is flagged iff some component's spread passes that component's threshold, and the accepted sums are
  * kept per component; the scalar instance is the code as it was. */
 template <bool VEC>
-__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __grid_constant__ ZmcCtlArgs c) {
+__device__ __forceinline__ void zmc_scatter_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
     __shared__ double smem[ZMC_CTL_THREADS];
     __shared__ zu32 warp_cnt[ZMC_CTL_THREADS / 32], warp_cnt_eq[ZMC_CTL_THREADS / 32];
     __shared__ zu64 run, run_eq;
     const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
     const zu32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    for (zu64 tile = bid; tile < n_tiles; tile += nb) {
         const ZmcTile T(c, tile);
         const zu64 G = T.G;
         const zu32 inst = c.cur.inst[G];
@@ -654,12 +714,14 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __gr
         }
     }
 }
+template <bool VEC>
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_scatter_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_scatter_kernel_body<VEC>(c, blockIdx.x, gridDim.x); }
 
 /* R7: value_b += sum of accepted mu ; var_b += sum of accepted s^2, one block per instance, over its tiles */
-__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_accumulate_kernel(const __grid_constant__ ZmcCtlArgs c) {
+__device__ __forceinline__ void zmc_accumulate_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
     __shared__ double smem[ZMC_CTL_THREADS];
     const zu64 nc = c.nc;
-    for (zu64 e = blockIdx.x; e < (zu64)c.n_inst * nc; e += gridDim.x) {      /* one block per (instance, component) */
+    for (zu64 e = bid; e < (zu64)c.n_inst * nc; e += nb) {      /* one block per (instance, component) */
         const zu64 b = e / nc, jc = e - b * nc;
         const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
         double am = 0.0, av = 0.0;
@@ -675,16 +737,25 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_accumulate_kernel(const _
         }
     }
 }
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_accumulate_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_accumulate_kernel_body(c, blockIdx.x, gridDim.x); }
+#endif
 
 /* result[b] = value_b ; result[n_inst + b] = sqrt(var_b)   (n_inst here = instances * components, R15) */
-__global__ void zmc_finalize_kernel(const double* value, const double* var, double* result, zu32 n_inst) {
-    for (zu64 b = (zu64)blockIdx.x * blockDim.x + threadIdx.x; b < n_inst; b += (zu64)gridDim.x * blockDim.x) {
+__device__ __forceinline__ void zmc_finalize_body(const double* value, const double* var, double* result, zu32 n_inst, zu32 bid, zu32 nb) {
+    for (zu64 b = (zu64)bid * blockDim.x + threadIdx.x; b < n_inst; b += (zu64)nb * blockDim.x) {
         result[b] = value[b];
         result[n_inst + b] = __dsqrt_rn(var[b]);
     }
 }
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void zmc_finalize_kernel(const double* value, const double* var, double* result, zu32 n_inst) {
+    zmc_finalize_body(value, var, result, n_inst, blockIdx.x, gridDim.x);
+}
+#endif
 
 /* debug: words of one unit's flat stream (R3) */
+#ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void zmc_words_kernel(const zu32* keys, zu32 inst, zu64 path_lo, zu32 path_hi, zu32 level, zu32 trial,
                                  zu64 first_word, zu64 n_words, zu32* out) {
     ZmcKeySchedule ks;
@@ -699,5 +770,6 @@ __global__ void zmc_words_kernel(const zu32* keys, zu32 inst, zu64 path_lo, zu32
         out[i] = (l == 0) ? w[0] : (l == 1) ? w[1] : (l == 2) ? w[2] : w[3];
     }
 }
+#endif
 
 #endif /* ZMC_CONTROL_CUH */

@@ -331,7 +331,10 @@ struct ZmcMapF64 {
         step[d] = __dmul_rn(width, 2.3283064365386963e-10);
     }
     __device__ __forceinline__ double x(int d, zu32 w) const {
-        return __dadd_rn(lo[d], __dmul_rn(__dadd_rn(__uint2double_rn(w), 0.5), step[d]));
+        /* (double)w + 0.5 without the conversion: bits (0x43300000 : w) are the double 2^52 + w, and (2^52 + w) - (2^52 - 0.5) is
+         * exact -- one DADD instead of I2F.F64.U32 (XU pipe, 8.5 clocks per warp-instruction) + DADD; the same value bit for bit */
+        const double wh = __dadd_rn(__hiloint2double(0x43300000, (zi32)w), -4503599627370495.5);
+        return __dadd_rn(lo[d], __dmul_rn(wh, step[d]));
     }
 };
 
@@ -928,8 +931,10 @@ __device__ __forceinline__ void zmc_unit(const ZmcSampleArgs& a, const F& f, con
  * parameters (constant bank), so the ten round keys live in uniform registers: 20 fewer registers
  * per thread and one register operand fewer on every Philox LOP3. */
 /* SQ (R13): also sum f^2 per unit, into partial_q. */
-template <class F, bool UKEY, bool SQ = false>
-__global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
+/* zmc_sample_items: the persistent item loop of one level, run by every warp of the grid until the level's counter is used up.
+ * It is the body of zmc_sample_kernel and, between two grid-wide barriers, of the single-launch tree kernel (zmc_tree.cuh). */
+template <class F, bool UKEY, bool SQ>
+__device__ __forceinline__ void zmc_sample_items(const ZmcSampleArgs& a) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG;
     const zu32 lane = threadIdx.x & 31u;
     ZmcLevelInfo* const info = a.info;
@@ -979,6 +984,11 @@ __global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sampl
             }
         }
     }
+}
+
+template <class F, bool UKEY, bool SQ = false>
+__global__ void __launch_bounds__(ZMC_BLOCK_THREADS, ZmcTune<F>::MINB) zmc_sample_kernel(const __grid_constant__ ZmcSampleArgs a) {
+    zmc_sample_items<F, UKEY, SQ>(a);
 }
 
 /* Debug kernel (parity tests P1): the first n samples of one unit through the same device functions. */

@@ -1,7 +1,8 @@
-/* zmc_inst.cu -- pre-compiled instances of the sampling kernel for one (precision, math mode,
+/* zmc_inst.cu -- pre-compiled instances of the sampling kernel (and of the single-launch tree kernel around it) for one (precision, math mode,
  * integrand) and every dimension 1..ZMC_AOT_MAX_DIM. build.py compiles this file once per
  * combination with -DZMC_INST_PREC= -DZMC_INST_MODE= -DZMC_INST_ID= (in parallel). */
-#include "zmc_device.cuh"
+#define ZMC_CONTROL_BODIES_ONLY
+#include "zmc_tree.cuh"
 #include "zmc_inst.h"
 
 #if !defined(ZMC_INST_PREC) || !defined(ZMC_INST_MODE) || !defined(ZMC_INST_ID)
@@ -15,6 +16,7 @@ static ZmcKernelEntry zmc_entry() {
     e.sample = (const void*)zmc_sample_kernel<F, false>;
     e.sample_ukey = (const void*)zmc_sample_kernel<F, true>;
     e.points = (const void*)zmc_points_kernel<F>;
+    e.tree = (const void*)zmc_tree_kernel<F>;
     return e;
 }
 
@@ -36,6 +38,6 @@ ZmcKernelEntry ZMC_LOOKUP_NAME(ZMC_INST_PREC, ZMC_INST_MODE, ZMC_INST_ID)(int di
         case 11: return zmc_entry<11>();
         case 12: return zmc_entry<12>();
     }
-    ZmcKernelEntry none = {nullptr, nullptr, nullptr};
+    ZmcKernelEntry none = {nullptr, nullptr, nullptr, nullptr};
     return none;
 }

@@ -9,6 +9,7 @@ struct ZmcKernelEntry {
     const void* sample;       /* zmc_sample_kernel<F, false>: per-item key (batched instances) */
     const void* sample_ukey;  /* zmc_sample_kernel<F, true>: one key for the whole launch (n_instances == 1) */
     const void* points;   /* zmc_points_kernel<F> */
+    const void* tree;     /* zmc_tree_kernel<F>: the whole tree search as one cooperative launch (zmc_tree.cuh) */
 };
 
 #define ZMC_DECLARE_LOOKUP(PREC, MODE, ID) ZmcKernelEntry zmc_lookup_##PREC##_##MODE##_##ID(int dim);

@@ -1,0 +1,112 @@
+"""The single-launch path (ZMC_OPT_SINGLE_LAUNCH, csrc/zmc_tree.cuh): one cooperative kernel for the whole tree search gives the
+same bits as the multi-launch path -- every per-(cell, trial) sum, (mu, s, tau), refined set and result -- on small trees
+(one block takes a sibling group through statistics, threshold and count), on sibling groups of several control tiles (the
+step-by-step order with grid barriers), with instances and a budget, on trees that end early; and it still matches the oracle."""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1902_07916_b200 import binding as B, workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+def _pair(w, **kw):
+    out = []
+    for single in (0, 1):
+        it = B.from_workload(w, keep_level_stats=True, single_launch=single, **kw)
+        it.run()
+        out.append(it)
+    return out
+
+
+def _same_bits(a, b, depth):
+    sa, sb = a.stats(), b.stats()
+    assert sa.kernel_launches > 1 and sb.kernel_launches == 1
+    for lev in range(1, depth + 1):
+        assert sa.level[lev - 1].n_cells == sb.level[lev - 1].n_cells
+        assert sa.level[lev - 1].n_flagged == sb.level[lev - 1].n_flagged
+        assert sa.level[lev - 1].n_refined == sb.level[lev - 1].n_refined
+        if sa.level[lev - 1].n_cells == 0:
+            continue
+        la, lb = a.level_cells(lev), b.level_cells(lev)
+        assert la.path == lb.path
+        for f in ("instance", "S", "mu", "s", "tau", "refined"):
+            np.testing.assert_array_equal(getattr(la, f), getattr(lb, f), err_msg="level %d %s" % (lev, f))
+    va, da = a.result()
+    vb, db = b.result()
+    np.testing.assert_array_equal(va, vb)
+    np.testing.assert_array_equal(da, db)
+
+
+def test_config1_single_launch_is_bit_identical_and_matches_the_oracle():
+    w = W.config1()
+    a, b = _pair(w)
+    _same_bits(a, b, w.depth)
+    ores = O.run(H.oracle_config(w), keep_cells=True)
+    assert H.compare_tree(b, ores, w) == 384
+    # default = auto: this problem (6.4e5 evaluations at level 1) takes the single launch
+    c = B.from_workload(w)
+    c.run()
+    assert c.stats().kernel_launches == 1
+    np.testing.assert_array_equal(c.result()[0], b.result()[0])
+    b.run()                                             # re-run on the same context
+    np.testing.assert_array_equal(c.result()[0], b.result()[0])
+    for it in (a, b, c):
+        it.close()
+
+
+def test_auto_keeps_large_problems_on_the_multi_launch_path():
+    w = W.config2(depth=2, budget=1).with_(n_samples=20000)        # 4096 * 5 * 2e4 = 4.1e8 evaluations at level 1
+    it = B.from_workload(w, max_cells_per_level=4096)
+    it.run()
+    st = it.stats()
+    assert st.kernel_launches == 2 + 6 * 2
+    it.close()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_batched_instances_with_budget(precision):
+    w = W.config4(n_instances=37).with_(g=3, n_samples=515, depth=3, max_groups_per_level=2, precision=precision)
+    a, b = _pair(w, max_cells_per_level=37 * 81 * 2)
+    _same_bits(a, b, 3)
+    ores = O.run(H.oracle_config(w), keep_cells=True)
+    H.compare_tree(b, ores, w)
+    a.close(); b.close()
+
+
+def test_three_tiles_per_group():
+    """k = 100^2 = 10000 cells: three 4096-cell control tiles per sibling group (the three-pass threshold, a grid barrier between
+    the passes)."""
+    w = W.Workload("solo_limit", 2, (0.0, 0.0), (10.0, 7.0), 100, 96, 3, 2, 1.0, 17, W.SIN_SUM, W.F32, max_groups_per_level=2)
+    a, b = _pair(w, max_cells_per_level=2 * 10000)
+    _same_bits(a, b, 2)
+    assert b.stats().level[1].n_cells == 20000
+    ores = O.run(H.oracle_config(w), keep_cells=True)
+    H.compare_tree(b, ores, w)
+    a.close(); b.close()
+
+
+def test_two_tiles_per_group_and_empty_levels():
+    """k = 70^2 = 4900 (two control tiles); a constant integrand flags nothing: levels 2 and 3 are empty."""
+    w = W.Workload("tiles_solo", 2, (0.0, 0.0), (1.0, 1.0), 70, 33, 4, 2, 0.5, 3, W.EXP_QUAD, W.F32,
+                   params=np.array([[1.0, 30.0, 0.4, 0.6]]), max_groups_per_level=1)
+    a, b = _pair(w, max_cells_per_level=4900)
+    _same_bits(a, b, 2)
+    a.close(); b.close()
+    w = W.Workload("const", 3, (0.0,) * 3, (1.0,) * 3, 3, 100, 3, 3, 1.0, 1, W.CONST, W.F64, params=np.array([[2.5]]))
+    a, b = _pair(w)
+    _same_bits(a, b, 3)
+    v, s = b.result()
+    assert abs(v[0] - 2.5) < 1e-12 and b.stats().level[1].n_cells == 0
+    a.close(); b.close()
+
+
+def test_forced_single_launch_where_it_does_not_exist_falls_back():
+    """R13 (sum-of-squares kernel) and user integrands have no tree kernel: the option is a preference, the run still works."""
+    w = W.config1()
+    it = B.from_workload(w, single_launch=1, spread=B.SPREAD_SAMPLES)
+    it.run()
+    assert it.stats().kernel_launches > 1
+    it.close()
