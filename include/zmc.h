@@ -80,7 +80,7 @@ enum {
                                          launch-bound problems (BASELINE.json configs[0]; PAPER.md:162-184 is about this per-call
                                          overhead). Same device functions, bit-identical results. 0 never, 1 whenever the kernel
                                          exists (pre-compiled integrands, ZMC_SPREAD_TRIALS, path-order budget), 2 = auto (default):
-                                         when level 1 has at most 1e8 evaluations. zmc_stats: kernel_launches 1, per-level times 0 */
+                                         when level 1 has at most 4e6 evaluations. zmc_stats: kernel_launches 1, per-level times 0 */
 };
 enum { ZMC_F64 = 0, ZMC_F32 = 1 };
 enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };

@@ -91,7 +91,9 @@ struct ZmcCtlArgs {
     zu64* excl_eq;
 };
 
-/* plan of one level: how the (cell, trial) units are cut into work items */
+/* plan of one level: how the (cell, trial) units are cut into work items. (Tried and not kept: choosing the number of chunks
+ * by a cost model "rounds x (item overhead + item length)" -- on BASELINE.json configs[0] level 2 as 1600 long items sampled in
+ * 28.7 us against 31.0 us as 11200 short ones, and the model's divisions cost the one planning thread 11 us.) */
 __device__ __forceinline__ void zmc_plan_level(ZmcLevelInfo& li, zu64 n_groups, const ZmcCtlArgs& c) {
     li.n_groups = n_groups;
     li.n_cells = n_groups * c.k;
@@ -114,6 +116,7 @@ __device__ __forceinline__ void zmc_plan_level(ZmcLevelInfo& li, zu64 n_groups, 
     li.work_ctr = 0;
     li.n_flagged = 0;
     li.n_refined = 0;
+    li.t_mark[0] = li.t_mark[1] = li.t_mark[2] = li.t_mark[3] = 0ull;
 }
 
 /* R3: Kd(seed, b) = words 0,1 of Philox(ctr = (b, 0, 0, 0x5A4D4321), key = (seed_lo, seed_hi)) */
@@ -145,6 +148,7 @@ __device__ __forceinline__ void zmc_init_kernel_body(const ZmcCtlArgs& c, const 
             ZmcLevelInfo z;
             z.n_groups = z.n_cells = z.n_items = z.work_ctr = z.n_flagged = z.n_refined = 0;
             z.n_chunks = 1; z.chunk_groups = c.sample_groups; z.trials_per_item = 1; z.reserved = 0;
+            z.t_mark[0] = z.t_mark[1] = z.t_mark[2] = z.t_mark[3] = 0ull;
             if (l != 1) c.info[l] = z;
         }
         ZmcLevelInfo li;
@@ -178,6 +182,13 @@ __device__ __forceinline__ void zmc_cell_stats_span(const ZmcCtlArgs& c, const z
         }
         const double VA = __dmul_rn(c.V, A);
         const double* p = c.partial + cell * (zu64)c.T * nch * nc + jc;
+        /* the cell's T * n_chunks partial sums are read one after the other below (a dependent chain of FP64 adds): ask for their
+         * cache lines first, all at once, so that the chain does not pay an L2 round trip per trial */
+        if (nch > 1u || c.T > 4u) {
+            const char* q0 = (const char*)p;
+            const zu64 bytes = (zu64)c.T * nch * nc * sizeof(double);
+            for (zu64 off = 0; off < bytes; off += 128ull) asm volatile("prefetch.global.L1 [%0];" ::"l"(q0 + off));
+        }
         double acc = 0.0;
         for (zu32 t = 0; t < c.T; ++t) {
             double S = p[(zu64)t * nch * nc];

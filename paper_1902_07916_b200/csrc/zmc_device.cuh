@@ -58,6 +58,9 @@ struct ZmcLevelInfo {
     zu32 trials_per_item; /* 1, or T on levels with many cells: one warp takes all trials of a cell, so that the item decoding
                              and the cell geometry are paid once per cell instead of once per trial (n_chunks == 1 then) */
     zu32 reserved;
+    /* single-launch path only (zmc_tree.cuh): %globaltimer (ns) as block 0 passes the level's grid barriers -- level begun,
+     * sampling done, statistics/thresholds done, control done: what zmc_stats reports as sample_ms / control_ms there */
+    zu64 t_mark[4];
 };
 
 struct ZmcSampleArgs {

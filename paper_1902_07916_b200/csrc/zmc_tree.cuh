@@ -37,6 +37,14 @@ struct ZmcTreeArgs {
 
 /* two 256-thread blocks per SM (128 registers) keep as many warps on the sampling phase as the multi-launch kernel has; FP64 at
  * high D would spill there */
+__device__ __forceinline__ void zmc_tree_mark(const ZmcCtlArgs& ca, zu32 level, int which) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        zu64 t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        ca.info[level].t_mark[which] = t;
+    }
+}
+
 template <class F> struct ZmcTreeTune { static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && F::D >= 7) ? 1 : 2; };
 
 template <class F>
@@ -55,8 +63,10 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS, ZmcTreeTune<F>::MINB) zmc_tre
         __syncthreads();
         if (threadIdx.x == 0) { sa = t.sample[level - 1]; ca = t.ctl[level - 1]; }
         __syncthreads();
+        zmc_tree_mark(ca, level, 0);
         zmc_sample_items<F, false, false>(sa);
         grid.sync();
+        zmc_tree_mark(ca, level, 1);
         const bool last = level >= t.L;
         const bool fused = ca.tpg == 1u;       /* a sibling group is one control tile: statistics, threshold and count by one block */
         if (fused) {
@@ -71,11 +81,13 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS, ZmcTreeTune<F>::MINB) zmc_tre
             zmc_threshold_pass_kernel_body<2>(ca, blockIdx.x, gridDim.x);
         }
         grid.sync();
+        zmc_tree_mark(ca, level, 2);
         if (fused && last) break;             /* the accepted sums are there: block 0 finishes below */
         if (blockIdx.x == 0) zmc_scan_kernel_body(ca);
         grid.sync();
         zmc_scatter_kernel_body<false>(ca, blockIdx.x, gridDim.x);
         grid.sync();
+        zmc_tree_mark(ca, level, 3);
         /* value += accepted sums: nobody needs it before the end, so block 0 does it while the others sample the next level */
         if (blockIdx.x == 0) zmc_accumulate_kernel_body(ca, 0u, 1u);
     }
@@ -87,6 +99,7 @@ __global__ void __launch_bounds__(ZMC_CTL_THREADS, ZmcTreeTune<F>::MINB) zmc_tre
         }
         __syncthreads();
         zmc_finalize_body(t.value, t.var, t.result, t.n_res, 0u, 1u);
+        zmc_tree_mark(ca, t.L, 3);
     }
 }
 

@@ -330,7 +330,7 @@ def test_graph_mode_is_bit_identical():
         ref = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 15)
         ref.run()
         rv, rs = ref.result()
-        it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 15, use_graph=True)
+        it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=1 << 15, use_graph=True, single_launch=0)    # these small trees would take the single launch
         for rep in range(3):
             it.run()
             v, s = it.result()

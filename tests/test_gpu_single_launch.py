@@ -58,7 +58,7 @@ def test_config1_single_launch_is_bit_identical_and_matches_the_oracle():
 
 
 def test_auto_keeps_large_problems_on_the_multi_launch_path():
-    w = W.config2(depth=2, budget=1).with_(n_samples=20000)        # 4096 * 5 * 2e4 = 4.1e8 evaluations at level 1
+    w = W.config2(depth=2, budget=1).with_(n_samples=2000)        # 4096 * 5 * 2000 = 4.1e7 evaluations at level 1
     it = B.from_workload(w, max_cells_per_level=4096)
     it.run()
     st = it.stats()
