@@ -95,19 +95,51 @@ def alu_peak_evals_per_s(dim, n_sm, sm_mhz):
     return n_sm * sm_mhz * 1e6 * 32.0 / clk_per_warp_eval
 
 
+def imad_wide_issued_per_eval(dim):
+    """IMAD.WIDE.U32 the shipped FP32 kernels issue per evaluation (SASS count, confirmed by ncu: profiles/r2_pipe_split.md).
+    Of a call's 20 multiplies the unit-constant ones are hoisted (M1*c2 of round 1, M0*c0 of round 2): 18 per call; with
+    P0_CARRY (D = 4, 6, 12) the first round's M0*c0 is a 64-bit addition as well: 17 per call."""
+    per_call = 17 if dim in (4, 6, 12) else 18
+    return per_call * calls_per_eval(dim)
+
+
+# FP32 instructions (scalar count) and XU conversions per evaluation of the built-in integrands in exact mode (DESIGN.md R8):
+# map D FFMA; SIN_SUM: D-1 FADD + 11 (zsin); EXP_QUAD: D (quadratic form) + 1 + 10 (zexp). One F2F.F64.F32 per sample on the XU pipe.
+def fp32_ops_per_eval(w):
+    if w.integrand == "sin_sum":
+        return w.dim + (w.dim - 1) + 11
+    if w.integrand == "exp_quad":
+        return w.dim + w.dim + 1 + 10
+    return 2 * w.dim
+
+
+def other_roofs(w, n_sm, sm_mhz):
+    """The roofs BASELINE.json's metric names, for the integrand's operation mix, next to the IMAD.WIDE roof that binds:
+    FP32: 128 lanes per SM per clock; XU (F2F.F64.F32, MUFU): one warp-instruction per 8.5 clocks per scheduler (measured,
+    profiles/r1_microbench.md) = 15.06 lanes per SM per clock."""
+    f = sm_mhz * 1e6
+    return {"fp32_fma_gevals_per_s": n_sm * 128.0 * f / fp32_ops_per_eval(w) / 1e9,
+            "xu_gevals_per_s": n_sm * 4 * 32.0 / 8.5 * f / 1.0 / 1e9,
+            "note": "evaluations/s if only that pipe were the limit (exact mode: %d FP32 instructions and 1 XU conversion per evaluation)" % fp32_ops_per_eval(w)}
+
+
 def traffic_from_profiles(workload, math):
     """DRAM bytes (read + write) per launch of the sampling kernel from the committed ncu --set full summary
     (profiles/traffic.csv): the mean over the launches captured for this workload, or None."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(path):
         return None
-    vals = []
+    vals, commits = [], set()
     for line in open(path):
         parts = [x.strip() for x in line.split(",")]
         if line.startswith("#") or len(parts) < 5 or parts[0] != workload or parts[1] != math:
             continue
         vals.append(float(parts[3]) + float(parts[4]))
-    return sum(vals) / len(vals) if vals else None
+        if len(parts) > 6:
+            commits.add(parts[6])
+    if not vals:
+        return None, None
+    return sum(vals) / len(vals), ",".join(sorted(commits))
 
 
 class ClockSampler:
@@ -270,7 +302,7 @@ def main():
 
     import numpy as np
     import torch
-    from paper_1902_07916_b200 import binding as B
+    from paper_1902_07916_b200 import binding as B, workloads as W
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -343,9 +375,16 @@ def main():
         pass
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = alu_peak_evals_per_s(w.dim, n_sm, sm_max)
-    traffic = traffic_from_profiles(args.workload, args.math)
+    traffic, traffic_commit = traffic_from_profiles(args.workload, args.math)
+    peak_issued = n_sm * sm_max * 1e6 * 32.0 / (4.0 * imad_wide_issued_per_eval(w.dim))
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s", "frac": achieved / peak,
+                "frac_algorithmic": achieved / peak,
+                # the same time against the multiplies the kernel really issues (FP32 built-ins): how busy they keep the FMA-heavy pipe
+                "frac_pipe": (achieved / peak_issued) if w.precision == "f32" else None,
+                "imad_wide_per_eval": {"algorithmic": PHILOX_IMAD_WIDE_PER_CALL * calls_per_eval(w.dim), "issued": imad_wide_issued_per_eval(w.dim)},
+                "other_roofs": other_roofs(w, n_sm, sm_max),
                 "traffic": traffic,
+                "traffic_source": ("profiles/traffic.csv: ncu --set full capture at commit %s" % traffic_commit) if traffic is not None else None,
                 "kernel": "zmc_sample_kernel", "launches_per_step": n_sample_launches, "avg_launch_ms": samp_ms / max(1, n_sample_launches),
                 "share_of_step": samp_ms / (st.total_ms if st.total_ms > 0 else ms_per_step),
                 "peak_basis": "IMAD.WIDE.U32 pipe: %d SMs x %.0f MHz (sm_max_mhz, %s) x 32 lanes / (20 IMAD.WIDE per Philox call x %.2f calls per eval x 1 clk)" %
@@ -415,8 +454,9 @@ def main():
                 itx.close()
             # BASELINE.json configs[0] is launch-bound (microseconds of arithmetic): kernel by kernel vs one CUDA graph
             w1 = wl["cfg1_sin3d_f64"]
-            for key, graph in (("cfg1_sin3d_f64", False), ("cfg1_sin3d_f64_graph", True)):
-                it1 = B.from_workload(w1, math=math, max_cells_per_level=capacity_for(w1), use_graph=graph)
+            # ... vs one cooperative launch for the whole tree (ZMC_OPT_SINGLE_LAUNCH; the default for a problem this small)
+            for key, graph, single in (("cfg1_sin3d_f64", False, None), ("cfg1_sin3d_f64_multi_launch", False, 0), ("cfg1_sin3d_f64_graph", True, 0)):
+                it1 = B.from_workload(w1, math=math, max_cells_per_level=capacity_for(w1), use_graph=graph, single_launch=single)
                 for _ in range(3):
                     it1.run(stream.cuda_stream)
                 it1.result()
@@ -426,8 +466,25 @@ def main():
                     it1.run(stream.cuda_stream)
                 g1.record(stream)
                 v1, s1 = it1.result()
-                line["time_to_result"][key] = {"ms": g0.elapsed_time(g1) / 20, "value": float(v1[0]), "std": float(s1[0])}
+                line["time_to_result"][key] = {"ms": g0.elapsed_time(g1) / 20, "value": float(v1[0]), "std": float(s1[0]),
+                                               "kernel_launches": int(it1.stats().kernel_launches)}
                 it1.close()
+            # SURVEY 8(f).4 / DESIGN.md R15: a vector-valued user integrand (NVRTC) -- C components from ONE sample stream, against C = 1
+            wv = W.vec_moments6d()
+            line["vector_valued"] = {"workload": wv.name, "note": wv.note}
+            for C_ in (1, 8):
+                itv = B.Integrator(wv.dim, wv.lower, wv.upper, wv.g, wv.n_samples, wv.trials, wv.depth, wv.sigma_multiplier, wv.seed)
+                itv.set_option(B.OPT_PRECISION, B.F32)
+                itv.set_integrand_source_vec(W.VEC_MOMENTS_SRC, W.VEC_MOMENTS_FN, C_, wv.params, 1)
+                itv.set_option(B.OPT_MAX_CELLS_PER_LEVEL, wv.k)
+                for _ in range(2):
+                    itv.run(stream.cuda_stream)
+                vv, sv = itv.result()
+                stv = itv.stats()
+                line["vector_valued"]["C%d" % C_] = {"ms": stv.total_ms, "points_per_s": stv.total_evals / (stv.total_ms * 1e-3),
+                                                     "component_evals_per_s": C_ * stv.total_evals / (stv.total_ms * 1e-3),
+                                                     "value0": float(vv[0][0]), "std0": float(sv[0][0])}
+                itv.close()
 
         if world == 1 and not args.no_cpu_baseline:
             units = max(1, int(2.0e8 // w.n_samples))

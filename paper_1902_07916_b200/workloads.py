@@ -117,3 +117,28 @@ def paper_table4_gauss9d() -> Workload:
     return Workload("paper_t4_gauss9d", 9, (-1.0,) * 9, (1.0,) * 9, 3, 10000, 5, 4, 4.0, 34, EXP_QUAD, F32,
                     params=gaussian_params(9, 0.01), max_cells_per_level=4 * 3 ** 9,
                     note="paper Table 4 (PAPER.md:202-216); f2, Eq. (2), D = 9")
+
+
+# ---------------------------------------------------------------- vector-valued user integrands (R15)
+# Inputs, not arithmetic of the method: CUDA device-function text handed to zmc_set_integrand_source_vec (and, `__device__`
+# defined away, to g++ for the oracle). f_j(x) = (p0 * sum_d x_d)^(j+1), j = 0 .. n_out-1: n_out "terms" that share one sample
+# stream -- the shape of the paper's application, an integrand of "several thousands terms".
+VEC_MOMENTS_FN = "moments8"
+VEC_MOMENTS_SRC = """
+template <class R> __device__ inline void moments8_t(const R* x, int dim, const R* p, int np, R* out, int n_out) {
+    R s = x[0];
+    for (int d = 1; d < dim; ++d) s = s + x[d];
+    R c = p[0] * s;
+    R v = c;
+    for (int j = 0; j < n_out; ++j) { out[j] = v; v = v * c; }
+}
+__device__ void moments8(const float* x, int dim, const float* p, int np, float* out, int n_out) { moments8_t<float>(x, dim, p, np, out, n_out); }
+__device__ void moments8(const double* x, int dim, const double* p, int np, double* out, int n_out) { moments8_t<double>(x, dim, p, np, out, n_out); }
+"""
+
+
+def vec_moments6d(n_components: int = 8) -> Workload:
+    """6-D, 4096 cells, 1e5 samples per cell, 5 trials, one level: BASELINE.json configs[1]'s sizes with the vector-valued integrand above
+    (integrand/params are placeholders here: the function is VEC_MOMENTS_SRC, its parameter p0 = 0.3)."""
+    return Workload("vec_moments6d_c%d" % n_components, 6, (0.0,) * 6, (1.0,) * 6, 4, 100000, 5, 1, 1.5, 6, CONST, F32,
+                    params=np.array([[0.3]]), note="DESIGN.md R15: %d components, one sample stream" % n_components)

@@ -66,11 +66,6 @@ SCALED_AXES = _templated("scaled_axes", """
     R b = t * x[1];
     out[1] = p[0] * b;""")
 
-# a 6-D oscillating family sharing one phase: f_j = (sum x)^j-like polynomial moments of s = sum_d x_d, j = 1..8
-# (Horner-free: each component one more multiply), the shape of "one sample stream, many terms" (PAPER.md:232)
-MOMENTS8 = _templated("moments8", """
-    R s = x[0];
-    for (int d = 1; d < dim; ++d) s = s + x[d];
-    R c = p[0] * s;
-    R v = c;
-    for (int j = 0; j < n_out; ++j) { out[j] = v; v = v * c; }""")
+# eight polynomial moments of s = p0 * sum_d x_d sharing one sample stream: the bench's vector-valued workload (an input recipe,
+# kept with the other workloads)
+from paper_1902_07916_b200.workloads import VEC_MOMENTS_SRC as MOMENTS8  # noqa: E402
