@@ -376,10 +376,10 @@ def main():
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = alu_peak_evals_per_s(w.dim, n_sm, sm_max)
     traffic, traffic_commit = traffic_from_profiles(args.workload, args.math)
-    peak_issued = n_sm * sm_max * 1e6 * 32.0 / (4.0 * imad_wide_issued_per_eval(w.dim))
+    peak_issued = n_sm * sm_max * 1e6 * 32.0 / (IMAD_WIDE_CLK_PER_WARP_INST_PER_SM * imad_wide_issued_per_eval(w.dim))
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s", "frac": achieved / peak,
                 "frac_algorithmic": achieved / peak,
-                # the same time against the multiplies the kernel really issues (FP32 built-ins): how busy they keep the FMA-heavy pipe
+                # the same time against the multiplies the kernel really issues (FP32 built-ins): the share of the time the FMA-heavy pipe spends on them
                 "frac_pipe": (achieved / peak_issued) if w.precision == "f32" else None,
                 "imad_wide_per_eval": {"algorithmic": PHILOX_IMAD_WIDE_PER_CALL * calls_per_eval(w.dim), "issued": imad_wide_issued_per_eval(w.dim)},
                 "other_roofs": other_roofs(w, n_sm, sm_max),
