@@ -164,74 +164,87 @@ __global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_init
 
 /* R5: S_t = sum of the chunk partials in chunk order ; I_t = ((V*A)*S_t)/(double)N ;
  * mu = (sum_t I_t)/T ; s = sqrt((sum_t (I_t-mu)^2)/T)  -- two-pass, population form. */
-/* the (cell, component) entries first, first + step, .. < last: one thread per entry */
-__device__ __forceinline__ void zmc_cell_stats_span(const ZmcCtlArgs& c, const zu64 first, const zu64 last, const zu64 step) {
+/* One block, batches of floor(256 / T) entries (an entry = a (cell, component)); entries [e_begin, e_end), batches b_first, b_first + b_step, ..
+ * One thread per (entry, trial) sums that trial's chunk partials (in chunk order) and forms I_t -- T independent loads and divisions side by side
+ * instead of one thread walking them as a chain; then the entry's first thread adds the T values in trial order. The arithmetic of every number is what
+ * a single thread would do, operation by operation (R5, R13). sh: 3 * ZMC_CTL_THREADS doubles of shared memory. */
+__device__ __forceinline__ void zmc_cell_stats_batches(const ZmcCtlArgs& c, const zu64 e_begin, const zu64 e_end, const zu64 b_first,
+                                                       const zu64 b_step, double* sh) {
     const ZmcLevelInfo& li = c.info[c.level];
     const zu32 nch = li.n_chunks;
     const double dN = (double)c.N, dT = (double)c.T;
-    zu64 bad = 0;
     const zu64 nc = c.nc;
-    /* one thread per (cell, component): component j of work item i is partial[i * nc + j] (R15); nc == 1: one thread per cell */
-    for (zu64 e = first; e < last; e += step) {
-        const zu64 cell = (nc == 1ull) ? e : e / nc;
-        const zu64 jc = e - cell * nc;
-        double A = 1.0;
-        if (c.prefactor_index >= 0) {
-            const zu32 inst = c.cur.inst[cell / c.k];
-            A = c.params[(zu64)inst * (zu64)c.ppi + (zu64)c.prefactor_index];
-        }
-        const double VA = __dmul_rn(c.V, A);
-        const double* p = c.partial + cell * (zu64)c.T * nch * nc + jc;
-        /* the cell's T * n_chunks partial sums are read one after the other below (a dependent chain of FP64 adds): ask for their
-         * cache lines first, all at once, so that the chain does not pay an L2 round trip per trial */
-        if (nch > 1u || c.T > 4u) {
-            const char* q0 = (const char*)p;
-            const zu64 bytes = (zu64)c.T * nch * nc * sizeof(double);
-            for (zu64 off = 0; off < bytes; off += 128ull) asm volatile("prefetch.global.L1 [%0];" ::"l"(q0 + off));
-        }
-        double acc = 0.0;
-        for (zu32 t = 0; t < c.T; ++t) {
-            double S = p[(zu64)t * nch * nc];
-            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]);
-            if (c.S) c.S[(cell * c.T + t) * nc + jc] = S;
-            acc = __dadd_rn(acc, __ddiv_rn(__dmul_rn(VA, S), dN));
-        }
-        const double mu = __ddiv_rn(acc, dT);
-        double sd;
-        if (c.spread == 0) {
-            double q = 0.0;
-            for (zu32 t = 0; t < c.T; ++t) {
-                double S = p[(zu64)t * nch * nc];
-                for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]);
-                const double d = __dadd_rn(__ddiv_rn(__dmul_rn(VA, S), dN), -mu);
-                q = __dadd_rn(q, __dmul_rn(d, d));
+    const zu32 T = c.T;
+    const zu32 epb = (zu32)ZMC_CTL_THREADS / T;          /* T <= 255: at least one entry per batch */
+    const zu32 le = threadIdx.x / T, t = threadIdx.x - le * T;
+    double* shI = sh;
+    double* shS = sh + ZMC_CTL_THREADS;
+    double* shQ = sh + 2 * ZMC_CTL_THREADS;
+    const zu64 n_batches = (e_end > e_begin) ? (e_end - e_begin + epb - 1) / epb : 0ull;
+    zu64 bad = 0;
+    for (zu64 b = b_first; b < n_batches; b += b_step) {
+        const zu64 e = e_begin + b * epb + le;
+        const bool live = le < epb && e < e_end;
+        double VA = 0.0;
+        if (live) {
+            const zu64 cell = (nc == 1ull) ? e : e / nc;
+            const zu64 jc = e - cell * nc;
+            double A = 1.0;
+            if (c.prefactor_index >= 0) {
+                const zu32 inst = c.cur.inst[cell / c.k];
+                A = c.params[(zu64)inst * (zu64)c.ppi + (zu64)c.prefactor_index];
             }
-            sd = __dsqrt_rn(__ddiv_rn(q, dT));
-        } else {
-            /* R13: Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples ; d = Qc - Sc^2/M, 0 unless d > Qc*2^-40 ;
-             * s = (V*A) * sqrt((d/M)/M), the standard error of mu. Scalar integrands only (nc == 1: the host refuses R13 otherwise) */
-            const double* pq = c.partial_q + cell * (zu64)c.T * nch;
-            double Sc = 0.0, Qc = 0.0;
-            for (zu32 t = 0; t < c.T; ++t) {
-                double S = p[(zu64)t * nch], Q = pq[(zu64)t * nch];
-                for (zu32 ch = 1; ch < nch; ++ch) { S = __dadd_rn(S, p[(zu64)t * nch + ch]); Q = __dadd_rn(Q, pq[(zu64)t * nch + ch]); }
-                if (c.Q) c.Q[cell * c.T + t] = Q;
-                Sc = __dadd_rn(Sc, S);
-                Qc = __dadd_rn(Qc, Q);
+            VA = __dmul_rn(c.V, A);
+            const zu64 unit = cell * (zu64)T + t;
+            const double* p = c.partial + unit * nch * nc + jc;
+            double S = p[0];
+            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)ch * nc]);
+            if (c.S) c.S[unit * nc + jc] = S;
+            shI[threadIdx.x] = __ddiv_rn(__dmul_rn(VA, S), dN);
+            if (c.spread != 0) {      /* R13 (nc == 1) */
+                const double* pq = c.partial_q + unit * nch;
+                double Q = pq[0];
+                for (zu32 ch = 1; ch < nch; ++ch) Q = __dadd_rn(Q, pq[ch]);
+                if (c.Q) c.Q[unit] = Q;
+                shS[threadIdx.x] = S;
+                shQ[threadIdx.x] = Q;
             }
-            const double M = __dmul_rn(dT, dN);
-            double d = __dadd_rn(Qc, -__ddiv_rn(__dmul_rn(Sc, Sc), M));
-            if (!(d > __dmul_rn(Qc, 9.094947017729282e-13))) d = 0.0;
-            sd = __dmul_rn(VA, __dsqrt_rn(__ddiv_rn(__ddiv_rn(d, M), M)));
         }
-        c.mu[e] = mu;
-        c.s[e] = sd;
-        if (!(fabs(mu) <= 1.7976931348623157e308) || !(fabs(sd) <= 1.7976931348623157e308)) ++bad;
+        __syncthreads();
+        if (live && t == 0u) {
+            const double* I = shI + le * T;
+            double acc = 0.0;
+            for (zu32 tt = 0; tt < T; ++tt) acc = __dadd_rn(acc, I[tt]);
+            const double mu = __ddiv_rn(acc, dT);
+            double sd;
+            if (c.spread == 0) {
+                double q = 0.0;
+                for (zu32 tt = 0; tt < T; ++tt) {
+                    const double d = __dadd_rn(I[tt], -mu);
+                    q = __dadd_rn(q, __dmul_rn(d, d));
+                }
+                sd = __dsqrt_rn(__ddiv_rn(q, dT));
+            } else {
+                /* R13: Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples ; d = Qc - Sc^2/M, 0 unless d > Qc*2^-40 ;
+                 * s = (V*A) * sqrt((d/M)/M), the standard error of mu. Scalar integrands only (the host refuses R13 otherwise) */
+                double Sc = 0.0, Qc = 0.0;
+                for (zu32 tt = 0; tt < T; ++tt) { Sc = __dadd_rn(Sc, shS[le * T + tt]); Qc = __dadd_rn(Qc, shQ[le * T + tt]); }
+                const double M = __dmul_rn(dT, dN);
+                double d = __dadd_rn(Qc, -__ddiv_rn(__dmul_rn(Sc, Sc), M));
+                if (!(d > __dmul_rn(Qc, 9.094947017729282e-13))) d = 0.0;
+                sd = __dmul_rn(VA, __dsqrt_rn(__ddiv_rn(__ddiv_rn(d, M), M)));
+            }
+            c.mu[e] = mu;
+            c.s[e] = sd;
+            if (!(fabs(mu) <= 1.7976931348623157e308) || !(fabs(sd) <= 1.7976931348623157e308)) ++bad;
+        }
+        __syncthreads();
     }
     if (bad) atomicAdd(c.nonfinite, bad);
 }
 __device__ __forceinline__ void zmc_cell_stats_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
-    zmc_cell_stats_span(c, (zu64)bid * blockDim.x + threadIdx.x, c.info[c.level].n_cells * (zu64)c.nc, (zu64)nb * blockDim.x);
+    __shared__ double sh[3 * ZMC_CTL_THREADS];
+    zmc_cell_stats_batches(c, 0ull, c.info[c.level].n_cells * (zu64)c.nc, bid, nb, sh);
 }
 #ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_cell_stats_kernel_body(c, blockIdx.x, gridDim.x); }
@@ -326,9 +339,9 @@ __device__ __forceinline__ void zmc_group_control_body(const ZmcCtlArgs& c, cons
     __shared__ zu64 smem_u[ZMC_CTL_THREADS];
     __shared__ double tau_sh[ZMC_DEV_MAX_COMPONENTS];
     const zu64 n_groups = c.info[c.level].n_groups;
+    __shared__ double sh[3 * ZMC_CTL_THREADS];
     for (zu64 G = bid; G < n_groups; G += nb) {
-        zmc_cell_stats_span(c, G * c.k + threadIdx.x, (G + 1ull) * c.k, blockDim.x);
-        __syncthreads();
+        zmc_cell_stats_batches(c, G * c.k, (G + 1ull) * c.k, 0ull, 1ull, sh);      /* ends with a __syncthreads */
         zmc_threshold_group(c, G, smem, smem_u, tau_sh);
         if (c.level >= c.L) {
             double acc_mu = 0.0, acc_var = 0.0;
