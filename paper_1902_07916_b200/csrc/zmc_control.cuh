@@ -89,6 +89,8 @@ struct ZmcCtlArgs {
     zu64* cnt_eq;           /* [tile] flagged cells with key == pivot */
     zu64* excl_gt;          /* [tile] exclusive prefixes over all tiles */
     zu64* excl_eq;
+    zu64* sel_state;        /* [instance][4] prefix, need, above, active: the radix select spread over the grid (few, large instances) */
+    zu64* sel_hist;         /* [instance][256] */
 };
 
 /* plan of one level: how the (cell, trial) units are cut into work items. (Tried and not kept: choosing the number of chunks
@@ -551,6 +553,74 @@ __global__ void __launch_bounds__(ZMC_SCAN_THREADS) zmc_select_kernel(const __gr
             __syncthreads();
         }
         if (threadIdx.x == 0) { c.piv[b] = sh_prefix; c.quota[b] = c.budget - sh_above; }
+    }
+}
+#endif
+
+/* The same selection for FEW, LARGE instances (a single-instance level of 10^8 cells must not be walked eight times by one block):
+ * one launch per step -- begin | 8 x (histogram by all tiles | pick one digit per instance). Integer logic only: the same pivot and quota. */
+#ifndef ZMC_CONTROL_BODIES_ONLY
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_select_begin_kernel(const __grid_constant__ ZmcCtlArgs c) {
+    for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
+        const zu64 g0 = c.gfirst[b], g1 = c.gend[b];
+        const zu64 cb = (g1 > g0) ? c.excl[g1 - 1] + c.cnt[g1 - 1] - c.excl[g0] : 0ull;
+        c.sel_hist[b * 256ull + threadIdx.x] = 0ull;
+        if (threadIdx.x == 0) {
+            zu64* st = c.sel_state + 4ull * b;
+            st[0] = 0ull; st[1] = c.budget; st[2] = 0ull;
+            st[3] = (cb > c.budget) ? 1ull : 0ull;
+            if (cb <= c.budget) { c.piv[b] = 0ull; c.quota[b] = ~0ull; }     /* nothing to cut (see zmc_select_kernel) */
+        }
+    }
+}
+
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_select_hist_kernel(const __grid_constant__ ZmcCtlArgs c, const int pass) {
+    __shared__ zu32 hist[256];
+    const zu64 n_tiles = c.info[c.level].n_groups * c.tpg;
+    const int shift = pass * 8;
+    for (zu64 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const ZmcTile T(c, tile);
+        const zu32 inst = c.cur.inst[T.G];
+        const zu64* st = c.sel_state + 4ull * inst;
+        if (st[3] == 0ull) continue;                     /* uniform over the block */
+        const zu64 prefix = st[0];
+        const double tau = c.tau[T.G];
+        __syncthreads();
+        hist[threadIdx.x] = 0u;
+        __syncthreads();
+        for (zu64 cell = T.c0 + threadIdx.x; cell < T.c1; cell += ZMC_CTL_THREADS) {
+            const double sj = c.s[cell];
+            if (sj > tau) {
+                const zu64 key = (zu64)__double_as_longlong(sj);
+                if (pass == 7 || (key >> (shift + 8)) == (prefix >> (shift + 8))) atomicAdd(&hist[(key >> shift) & 255ull], 1u);
+            }
+        }
+        __syncthreads();
+        const zu32 h = hist[threadIdx.x];
+        if (h) atomicAdd((unsigned long long*)&c.sel_hist[inst * 256ull + threadIdx.x], (unsigned long long)h);
+    }
+}
+
+__global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_select_pick_kernel(const __grid_constant__ ZmcCtlArgs c, const int pass) {
+    __shared__ zu64 h[256];
+    for (zu64 b = blockIdx.x; b < c.n_inst; b += gridDim.x) {
+        zu64* st = c.sel_state + 4ull * b;
+        __syncthreads();
+        h[threadIdx.x] = c.sel_hist[b * 256ull + threadIdx.x];
+        c.sel_hist[b * 256ull + threadIdx.x] = 0ull;     /* ready for the next pass */
+        __syncthreads();
+        if (threadIdx.x == 0 && st[3] != 0ull) {
+            zu64 cum = 0, need = st[1];
+            int digit = 0;
+            for (int dgt = 255; dgt >= 0; --dgt) {
+                if (cum + h[dgt] >= need) { digit = dgt; break; }
+                cum += h[dgt];
+            }
+            st[1] = need - cum;
+            st[2] += cum;
+            st[0] |= (zu64)digit << (pass * 8);
+            if (pass == 0) { c.piv[b] = st[0]; c.quota[b] = c.budget - st[2]; }
+        }
     }
 }
 #endif
