@@ -378,6 +378,9 @@ def _vec_lib():
         L.orc_vec_level_counts.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.orc_vec_level_cells.argtypes = [C.c_void_p, C.c_int, u32p, u64p, u32p, dp, dp, dp, C.POINTER(C.c_uint8), dp]
         L.orc_vec_level_cells.restype = C.c_int64
+        L.orc_vec_level_sumsq.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_vec_level_sumsq.restype = C.c_int64
+        L.orc_vec_unit_sums_sq.argtypes = [C.POINTER(_Cfg), C.c_int, USER_F64, USER_F32, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, dp, dp]
         L._vec_ready = True
     return L
 
@@ -398,6 +401,19 @@ def vec_unit_sums(cfg: Config, n_components, fns, instance, path, level, coords,
     if rc != 0:
         raise ValueError("oracle: bad config")
     return S
+
+
+def vec_unit_sums_sq(cfg: Config, n_components, fns, instance, path, level, coords, trial):
+    """R13 + R15: (S, Q), the n_components sums of f and of f^2 of one (cell, trial) unit."""
+    cc = np.ascontiguousarray(coords, dtype=np.uint32)
+    S, Q = np.zeros(n_components), np.zeros(n_components)
+    c = cfg.c()
+    f64, f32 = _fn_args(fns)
+    rc = _vec_lib().orc_vec_unit_sums_sq(C.byref(c), n_components, f64, f32, instance, path & (2**64 - 1), path >> 64, level,
+                                         _u32p(cc), trial, _dp(S), _dp(Q))
+    if rc != 0:
+        raise ValueError("oracle: bad config")
+    return S, Q
 
 
 def run_vec(cfg: Config, n_components, fns, keep_cells: bool = False) -> Result:
@@ -432,6 +448,10 @@ def run_vec(cfg: Config, n_components, fns, keep_cells: bool = False) -> Result:
                                       _dp(mu), _dp(s), _dp(tau), ref.ctypes.data_as(C.POINTER(C.c_uint8)), _dp(S))
                 rec.instance, rec.mu, rec.s, rec.tau, rec.refined, rec.S = inst, mu, s, tau, ref, S
                 rec.path = [int(phi[i]) << 64 | int(plo[i]) for i in range(n)]
+                if cfg.spread == SPREAD_SAMPLES:
+                    Q = np.zeros((n, cfg.trials, nc))
+                    L.orc_vec_level_sumsq(h, lev, _dp(Q))
+                    rec.Q = Q
             levels.append(rec)
         return Result(value, std, levels, L.orc_vec_total_evals(h))
     finally:

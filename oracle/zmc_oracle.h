@@ -114,13 +114,16 @@ int64_t orc_level_sumsq(const orc_result*, int level, double* Q);
 
 /* ---- R15: vector-valued user integrands (zmc_oracle_vec.cpp). The user function is an input of the method: it writes
  * n_out components of f at the point x (the FP64 or the FP32 arithmetic, by cfg->precision). cfg->integrand is ignored;
- * group scope, breadth-first, spread from the trials, path-order budget only. ---- */
+ * group scope, breadth-first, path-order budget only; the spread from the trials (R5) or, per component, from the samples (R13). ---- */
 typedef void (*orc_user_f64)(const double* x, int dim, const double* p, int np, double* out, int n_out);
 typedef void (*orc_user_f32)(const float* x, int dim, const float* p, int np, float* out, int n_out);
 typedef struct orc_vec_result orc_vec_result;
 /* S[j] = sum_s (double) f_j(x_s) of one (cell, trial) unit, j = 0 .. n_components-1 */
 int orc_vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
                       uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S);
+/* R13: the same unit, also Q[j] = sum_s f_j(x_s)^2 */
+int orc_vec_unit_sums_sq(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
+                         uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S, double* Q);
 orc_vec_result* orc_run_vec(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, int keep_cells);
 void orc_vec_free(orc_vec_result*);
 const char* orc_vec_error(const orc_vec_result*);
@@ -129,6 +132,7 @@ int orc_vec_levels(const orc_vec_result*);
 uint64_t orc_vec_total_evals(const orc_vec_result*);
 void orc_vec_level_counts(const orc_vec_result*, int level, int64_t* n_cells, int64_t* n_refined, int64_t* n_truncated);
 /* mu, s, tau: [cells * C]; S: [cells * T * C] (trial-major, component fastest); any pointer may be NULL */
+int64_t orc_vec_level_sumsq(const orc_vec_result*, int level, double* Q);   /* R13: [cells * T * C] */
 int64_t orc_vec_level_cells(const orc_vec_result*, int level, uint32_t* instance, uint64_t* path_lo, uint32_t* path_hi,
                             double* mu, double* s, double* tau, uint8_t* refined, double* S);
 

@@ -8,6 +8,7 @@
  *
  *   S_j(c,t) = sum_s (double) f_j(x_s)                                                  (R5, per component)
  *   (mu_j(c), s_j(c)) = orc_cell_stats(S_j(c, .))                                      (R5)
+ *                       or, with R13, orc_cell_stats_samples(S_j(c, .), Q_j(c, .)), Q_j(c,t) = sum_s f_j(x_s)^2
  *   tau_j(G) = orc_threshold(s_j over the k cells of sibling group G)                  (R6, per component)
  *   cell c of group G is flagged iff level < L and s_j(c) > tau_j(G) for SOME j        (R7 with "any component")
  *   budget B > 0: per instance and level the first B flagged cells in path order       (R12)
@@ -44,6 +45,7 @@ struct orc_vec_result {
         std::vector<uint32_t> path_hi;
         std::vector<double> mu, s, tau;           /* [cell*C + j] */
         std::vector<double> S;                    /* [(cell*T + t)*C + j] */
+        std::vector<double> Q;                    /* R13: sums of squares, same layout */
         std::vector<uint8_t> refined;
     };
     std::vector<Level> levels;
@@ -76,8 +78,8 @@ Cell child_of(const Cell& parent, int64_t j, int D, int g, int64_t k) {
 extern "C" {
 
 /* S[j] = sum over the unit's N samples of (double) f_j(x_s); sample s takes words s*D .. s*D+D-1 (R3), the point is R4's */
-int orc_vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
-                      uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S) {
+static int vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
+                         uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S, double* Q) {
     const int D = cfg->dim, C = n_components;
     if (D < 1 || D > 64 || C < 1 || C > 64) return -1;
     if (cfg->precision == ORC_F64 ? !f64 : !f32) return -1;
@@ -87,6 +89,7 @@ int orc_vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64,
     std::vector<float> pf((size_t)cfg->params_per_instance + 1);
     for (int i = 0; i < cfg->params_per_instance; ++i) pf[i] = (float)p[i];
     for (int j = 0; j < C; ++j) S[j] = 0.0;
+    if (Q) for (int j = 0; j < C; ++j) Q[j] = 0.0;
     std::vector<uint32_t> words((size_t)D);
     for (uint64_t s = 0; s < cfg->n_samples; ++s) {
         orc_unit_words(cfg->seed, instance, path_lo, path_hi, level, trial, s * (uint64_t)D, (uint64_t)D, words.data());
@@ -95,14 +98,26 @@ int orc_vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64,
             for (int d = 0; d < D; ++d) x[d] = orc_map_f64(words[d], lo[d], width[d]);
             f64(x, D, p, cfg->params_per_instance, out, C);
             for (int j = 0; j < C; ++j) S[j] = S[j] + out[j];
+            if (Q) for (int j = 0; j < C; ++j) { const double ff = out[j] * out[j]; Q[j] = Q[j] + ff; }      /* R13: product rounded, then added */
         } else {
             float x[64], out[64];
             for (int d = 0; d < D; ++d) x[d] = orc_map_f32(words[d], lo[d], width[d], 0.0);
             f32(x, D, pf.data(), cfg->params_per_instance, out, C);
             for (int j = 0; j < C; ++j) S[j] = S[j] + (double)out[j];
+            if (Q) for (int j = 0; j < C; ++j) { const double fd = (double)out[j]; const double ff = fd * fd; Q[j] = Q[j] + ff; }
         }
     }
     return 0;
+}
+
+int orc_vec_unit_sums(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
+                      uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S) {
+    return vec_unit_sums(cfg, n_components, f64, f32, instance, path_lo, path_hi, level, coords, trial, S, nullptr);
+}
+/* R13: the same unit, also Q[j] = sum_s f_j(x_s)^2 */
+int orc_vec_unit_sums_sq(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, uint32_t instance,
+                         uint64_t path_lo, uint32_t path_hi, int level, const uint32_t* coords, int trial, double* S, double* Q) {
+    return vec_unit_sums(cfg, n_components, f64, f32, instance, path_lo, path_hi, level, coords, trial, S, Q);
 }
 
 orc_vec_result* orc_run_vec(const orc_config* cfg, int n_components, orc_user_f64 f64, orc_user_f32 f32, int keep_cells) {
@@ -111,8 +126,9 @@ orc_vec_result* orc_run_vec(const orc_config* cfg, int n_components, orc_user_f6
         cfg->depth > 15 || cfg->n_samples < 1 || cfg->n_instances < 1) { R->err = "bad config"; return R; }
     if (n_components < 1 || n_components > 64) { R->err = "n_components out of range (1..64)"; return R; }
     if (cfg->precision == ORC_F64 ? !f64 : !f32) { R->err = "no user function for this precision"; return R; }
-    if (cfg->threshold_scope != ORC_SCOPE_GROUP || cfg->traversal != ORC_BFS || cfg->spread != ORC_SPREAD_TRIALS ||
-        cfg->budget_order != ORC_BUDGET_PATH_ORDER) { R->err = "vector-valued runs: group scope, BFS, spread from trials, path-order budget only"; return R; }
+    if (cfg->threshold_scope != ORC_SCOPE_GROUP || cfg->traversal != ORC_BFS || cfg->budget_order != ORC_BUDGET_PATH_ORDER) {
+        R->err = "vector-valued runs: group scope, BFS, path-order budget only"; return R; }
+    const bool from_samples = cfg->spread == ORC_SPREAD_SAMPLES;      /* R13 per component */
     const int D = cfg->dim, g = cfg->g, T = cfg->trials, L = cfg->depth, C = n_components;
     long double bits = (long double)L * (long double)D * std::log2((long double)g);
     if (bits > 80.0L) { R->err = "path exceeds 80 bits"; return R; }
@@ -132,22 +148,27 @@ orc_vec_result* orc_run_vec(const orc_config* cfg, int n_components, orc_user_f6
         R->levels_done = level;
         orc_vec_result::Level& LS = R->levels[level - 1];
         const size_t ng = parents.size(), n = ng * (size_t)k;
-        std::vector<double> mu(n * C), s(n * C), S(n * (size_t)T * C);
+        std::vector<double> mu(n * C), s(n * C), S(n * (size_t)T * C), Q(from_samples ? n * (size_t)T * C : 0);
         /* every cell: T trials, C sums each, then (mu_j, s_j) by R5 */
         for (size_t G = 0; G < ng; ++G)
             for (int64_t j = 0; j < k; ++j) {
                 const Cell c = child_of(parents[G], j, D, g, k);
                 const size_t i = G * (size_t)k + (size_t)j;
                 for (int t = 0; t < T; ++t)
-                    orc_vec_unit_sums(cfg, C, f64, f32, c.instance, (uint64_t)c.path, (uint32_t)(c.path >> 64), level,
-                                      c.coords.data(), t, &S[(i * (size_t)T + (size_t)t) * C]);
+                    vec_unit_sums(cfg, C, f64, f32, c.instance, (uint64_t)c.path, (uint32_t)(c.path >> 64), level, c.coords.data(), t,
+                                  &S[(i * (size_t)T + (size_t)t) * C], from_samples ? &Q[(i * (size_t)T + (size_t)t) * C] : nullptr);
                 R->evals += (uint64_t)T * cfg->n_samples;
                 double lo[64], width[64], V;
                 orc_cell_geometry(D, cfg->lower, cfg->upper, g, level, c.coords.data(), lo, width, &V);
-                std::vector<double> St((size_t)T);
+                std::vector<double> St((size_t)T), Qt((size_t)T);
                 for (int q = 0; q < C; ++q) {
                     for (int t = 0; t < T; ++t) St[t] = S[(i * (size_t)T + (size_t)t) * C + q];
-                    orc_cell_stats(St.data(), T, V, 1.0, cfg->n_samples, nullptr, &mu[i * C + q], &s[i * C + q]);
+                    if (from_samples) {
+                        for (int t = 0; t < T; ++t) Qt[t] = Q[(i * (size_t)T + (size_t)t) * C + q];
+                        orc_cell_stats_samples(St.data(), Qt.data(), T, V, 1.0, cfg->n_samples, &mu[i * C + q], &s[i * C + q]);
+                    } else {
+                        orc_cell_stats(St.data(), T, V, 1.0, cfg->n_samples, nullptr, &mu[i * C + q], &s[i * C + q]);
+                    }
                 }
             }
         /* R6 per component and sibling group */
@@ -196,6 +217,7 @@ orc_vec_result* orc_run_vec(const orc_config* cfg, int n_components, orc_user_f6
                     LS.refined.push_back(refine[i] ? 1 : 0);
                     for (int q = 0; q < C; ++q) { LS.mu.push_back(mu[i * C + q]); LS.s.push_back(s[i * C + q]); LS.tau.push_back(tau[G * C + q]); }
                     for (size_t e = 0; e < (size_t)T * C; ++e) LS.S.push_back(S[i * (size_t)T * C + e]);
+                    if (from_samples) for (size_t e = 0; e < (size_t)T * C; ++e) LS.Q.push_back(Q[i * (size_t)T * C + e]);
                 }
             }
         parents.swap(next);
@@ -235,6 +257,13 @@ int64_t orc_vec_level_cells(const orc_vec_result* r, int level, uint32_t* instan
     }
     if (S) for (size_t i = 0; i < ls.S.size(); ++i) S[i] = ls.S[i];
     return (int64_t)n;
+}
+
+/* R13: per-(cell, trial, component) sums of squares of one level, [cells*T*C]; nothing unless spread = samples and keep_cells */
+int64_t orc_vec_level_sumsq(const orc_vec_result* r, int level, double* Q) {
+    const orc_vec_result::Level& ls = r->levels[level - 1];
+    if (Q) for (size_t i = 0; i < ls.Q.size(); ++i) Q[i] = ls.Q[i];
+    return (int64_t)ls.Q.size();
 }
 
 }  /* extern "C" */

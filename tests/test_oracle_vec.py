@@ -151,6 +151,67 @@ def test_vector_driver_rejects_what_it_does_not_define():
     fns = O.compile_user_fn(VS.POLY4, "poly4")
     with pytest.raises(ValueError):
         O.run_vec(cfg, 0, fns)
-    cfg.spread = O.SPREAD_SAMPLES
+    cfg.budget_order = O.BUDGET_LARGEST_SPREAD
     with pytest.raises(ValueError):
         O.run_vec(cfg, 4, fns)
+
+
+# ------------------------------------------------------------ R13 per component (spread from the samples)
+@pytest.mark.parametrize("precision", [O.F64, O.F32])
+def test_spread_from_samples_one_component_is_the_scalar_driver_bit_for_bit(precision):
+    p = np.array([[0.3, 1.0, -2.0, 0.5]])
+    cfg = _cfg(params=p, precision=precision, integrand=O.LINEAR, lower=[0, -1, 2], upper=[1, 1, 2.5], m=0.5)
+    cfg.spread = O.SPREAD_SAMPLES
+    ref = O.run(cfg, keep_cells=True)
+    vec = O.run_vec(cfg, 1, O.compile_user_fn(VS.LINEAR1, "lin1"), keep_cells=True)
+    assert len(ref.levels) == len(vec.levels) and ref.levels[0].n_refined > 0
+    for a, b in zip(ref.levels, vec.levels):
+        np.testing.assert_array_equal(a.S, b.S[:, :, 0])
+        np.testing.assert_array_equal(a.Q, b.Q[:, :, 0])
+        np.testing.assert_array_equal(a.mu, b.mu[:, 0])
+        np.testing.assert_array_equal(a.s, b.s[:, 0])
+        np.testing.assert_array_equal(a.tau, b.tau[:, 0])
+        np.testing.assert_array_equal(a.refined, b.refined)
+    assert ref.value[0] == vec.value[0, 0] and ref.std[0] == vec.std[0, 0]
+
+
+def test_spread_from_samples_per_component_against_numpy():
+    """Every component's cell spread = V * sqrt(var(f_j over the cell's T*N samples) / (T*N)), recomputed with numpy from the
+    scalar oracle's points; sums of squares = the formulas squared at those points; a constant component has spread exactly 0."""
+    cfg = _cfg(lower=[0, 0, -1], upper=[1, 2, 1], n=300, T=4, depth=1, params=np.array([[0.0]]))
+    cfg.spread = O.SPREAD_SAMPLES
+    fns = O.compile_user_fn(VS.POLY4, "poly4")
+    r = O.run_vec(cfg, 4, fns, keep_cells=True)
+    L1 = r.levels[0]
+    V = (1.0 / 3) * (2.0 / 3) * (2.0 / 3)
+    for cell in (0, 13, 26):
+        path, coords = O.path_coords(3, 3, [cell])
+        vals = []
+        for t in range(4):
+            x, _ = O.unit_points(cfg, 0, path, 1, coords, t, 300)
+            f = np.stack([x[:, 0] * x[:, 1], x[:, 2] ** 2, np.full(300, 3.0), x[:, 0] + x[:, 1] * x[:, 2]], axis=1)
+            vals.append(f)
+            S, Q = O.vec_unit_sums_sq(cfg, 4, fns, 0, path, 1, coords, t)
+            np.testing.assert_allclose(S, f.sum(axis=0), rtol=1e-13)
+            np.testing.assert_allclose(Q, (f * f).sum(axis=0), rtol=1e-13)
+            np.testing.assert_allclose(L1.Q[cell, t], Q, rtol=0, atol=0)
+        allf = np.concatenate(vals, axis=0)
+        want = V * np.sqrt(allf.var(axis=0) / allf.shape[0])
+        np.testing.assert_allclose(L1.s[cell, [0, 1, 3]], want[[0, 1, 3]], rtol=1e-9)
+        assert L1.s[cell, 2] == 0.0
+    assert r.std[0, 2] == 0.0
+
+
+def test_spread_from_samples_gives_a_one_sigma_error_per_component():
+    """z = (value - closed form) / std over seeds: mean ~ 0 and variance ~ 1 for every non-constant component (R13's claim)."""
+    closed = np.array([2.0, 4.0 / 3.0, 12.0, 2.0])
+    fns = O.compile_user_fn(VS.POLY4, "poly4")
+    z = []
+    for seed in range(60):
+        cfg = _cfg(lower=[0, 0, -1], upper=[1, 2, 1], n=60, T=2, depth=1, seed=1000 + seed, g=2)
+        cfg.spread = O.SPREAD_SAMPLES
+        r = O.run_vec(cfg, 4, fns)
+        z.append((r.value[0, [0, 1, 3]] - closed[[0, 1, 3]]) / r.std[0, [0, 1, 3]])
+    z = np.array(z)
+    assert np.all(np.abs(z.mean(axis=0)) < 0.45)
+    assert np.all((z.var(axis=0) > 0.55) & (z.var(axis=0) < 1.6))
