@@ -131,8 +131,9 @@ int zmc_set_integrand_source(zmc_ctx* ctx, const char* cuda_src, const char* fn_
  * which writes out[0 .. n_out), n_out = n_components. Each component gets its own per-cell (mu, s) and per-group threshold; a cell is
  * refined iff SOME component's s exceeds that component's threshold; zmc_result then returns n_instances * n_components values and
  * stds, [instance][component], and the per-cell arrays of zmc_level_cells* carry C entries per cell (mu, s, tau: [cell*C + j];
- * S: [(cell*T + t)*C + j]). Compiled during this call like zmc_set_integrand_source. ZMC_ERR_STATE if ZMC_SPREAD_SAMPLES is in force,
- * or ZMC_BUDGET_LARGEST_SPREAD with C > 1 (not defined for several components); ZMC_ERR_RANGE for C outside 1..16. */
+ * S: [(cell*T + t)*C + j]). Compiled during this call like zmc_set_integrand_source. ZMC_SPREAD_SAMPLES applies per component
+ * (R13, R15). ZMC_ERR_STATE if ZMC_BUDGET_LARGEST_SPREAD is in force with C > 1 (not defined for several components);
+ * ZMC_ERR_RANGE for C outside 1..16. */
 int zmc_set_integrand_source_vec(zmc_ctx* ctx, const char* cuda_src, const char* fn_name, int n_components, const double* params,
                                  int params_per_instance, int n_instances);
 
@@ -211,7 +212,8 @@ int zmc_level_cells_range(zmc_ctx* ctx, int level, uint64_t first_cell, uint64_t
                           double* S);
 
 /* Per-(cell, trial) sums of f^2 of one level, Q[c*T + t], FP64 (R13); needs ZMC_OPT_KEEP_LEVEL_STATS and
- * ZMC_SPREAD_SAMPLES. Q [host] capacity*T doubles, capacity >= the level's cell count. */
+ * ZMC_SPREAD_SAMPLES. Q [host] capacity*T doubles (capacity*T*n_components, Q[(c*T + t)*C + j], for a vector-valued integrand),
+ * capacity >= the level's cell count. */
 int zmc_level_sumsq(zmc_ctx* ctx, int level, uint64_t capacity, double* Q);
 
 /* Raw generator access for parity tests (R1, R3): n_words words of the flat stream of unit

@@ -261,7 +261,7 @@ class Integrator:
         return LevelCells(inst, path, mu, s, tau, ref, S)
 
     def level_sumsq(self, level: int, n_cells: int) -> np.ndarray:
-        Q = np.zeros((n_cells, self.trials))
+        Q = np.zeros(self._cshape(n_cells, self.trials))
         self._check(self._L.zmc_level_sumsq(self._h, level, n_cells, _dp(Q)))
         return Q
 

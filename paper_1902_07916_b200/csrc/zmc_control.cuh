@@ -203,11 +203,11 @@ __device__ __forceinline__ void zmc_cell_stats_batches(const ZmcCtlArgs& c, cons
             for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[(zu64)ch * nc]);
             if (c.S) c.S[unit * nc + jc] = S;
             shI[threadIdx.x] = __ddiv_rn(__dmul_rn(VA, S), dN);
-            if (c.spread != 0) {      /* R13 (nc == 1) */
-                const double* pq = c.partial_q + unit * nch;
+            if (c.spread != 0) {      /* R13, per component */
+                const double* pq = c.partial_q + unit * nch * nc + jc;
                 double Q = pq[0];
-                for (zu32 ch = 1; ch < nch; ++ch) Q = __dadd_rn(Q, pq[ch]);
-                if (c.Q) c.Q[unit] = Q;
+                for (zu32 ch = 1; ch < nch; ++ch) Q = __dadd_rn(Q, pq[(zu64)ch * nc]);
+                if (c.Q) c.Q[unit * nc + jc] = Q;
                 shS[threadIdx.x] = S;
                 shQ[threadIdx.x] = Q;
             }
@@ -228,7 +228,7 @@ __device__ __forceinline__ void zmc_cell_stats_batches(const ZmcCtlArgs& c, cons
                 sd = __dsqrt_rn(__ddiv_rn(q, dT));
             } else {
                 /* R13: Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples ; d = Qc - Sc^2/M, 0 unless d > Qc*2^-40 ;
-                 * s = (V*A) * sqrt((d/M)/M), the standard error of mu. Scalar integrands only (the host refuses R13 otherwise) */
+                 * s = (V*A) * sqrt((d/M)/M), the standard error of mu (of each component's mu, R15) */
                 double Sc = 0.0, Qc = 0.0;
                 for (zu32 tt = 0; tt < T; ++tt) { Sc = __dadd_rn(Sc, shS[le * T + tt]); Qc = __dadd_rn(Qc, shQ[le * T + tt]); }
                 const double M = __dmul_rn(dT, dN);

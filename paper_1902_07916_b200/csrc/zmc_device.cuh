@@ -845,13 +845,17 @@ __device__ __forceinline__ void zmc_full_groups(const F& f, const ZmcKeySchedule
 /* R15: one unit of a vector-valued integrand -- the same word stream and the same points as a scalar unit, NC FP64 sums,
  * stored component-fastest at partial[out * NC + j]. One accumulator per component and lane (the user function, not the
  * generator, sets the pace here), plain Philox calls. */
-template <class F>
+template <class F, bool SQ>
 __device__ __forceinline__ void zmc_unit_vec(const ZmcSampleArgs& a, const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc,
                                              zu32 lane, zu32 gb, zu32 ge, zu32 gfe, zu32 full_groups, zu32 tail, zu64 out) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG, NC = F::NC;
-    double acc[NC];
+    double acc[NC], accq[SQ ? NC : 1];      /* SQ (R13 per component): sums of f_j^2 as well */
 #pragma unroll
     for (int j = 0; j < NC; ++j) acc[j] = 0.0;
+    if (SQ) {
+#pragma unroll
+        for (int j = 0; j < (SQ ? NC : 1); ++j) accq[j] = 0.0;
+    }
     for (zu32 gi = gb + lane; gi < gfe; gi += 32u) {
         zu32 w[4 * CG];
 #pragma unroll
@@ -862,6 +866,10 @@ __device__ __forceinline__ void zmc_unit_vec(const ZmcSampleArgs& a, const F& f,
             f.evalv(&w[s * D], o, nullptr);
 #pragma unroll
             for (int j = 0; j < NC; ++j) acc[j] = __dadd_rn(acc[j], o[j]);
+            if (SQ) {
+#pragma unroll
+                for (int j = 0; j < (SQ ? NC : 1); ++j) accq[j] = zmc_sq_add<F>(accq[j], o[j]);
+            }
         }
     }
     if (tail != 0u && ge > full_groups && lane == 0u) {
@@ -876,6 +884,10 @@ __device__ __forceinline__ void zmc_unit_vec(const ZmcSampleArgs& a, const F& f,
                 f.evalv(&w[s * D], o, nullptr);
 #pragma unroll
                 for (int j = 0; j < NC; ++j) acc[j] = __dadd_rn(acc[j], o[j]);
+                if (SQ) {
+#pragma unroll
+                    for (int j = 0; j < (SQ ? NC : 1); ++j) accq[j] = zmc_sq_add<F>(accq[j], o[j]);
+                }
             }
     }
 #pragma unroll
@@ -885,6 +897,15 @@ __device__ __forceinline__ void zmc_unit_vec(const ZmcSampleArgs& a, const F& f,
         for (int off = 16; off > 0; off >>= 1) sum = __dadd_rn(sum, __shfl_down_sync(0xFFFFFFFFu, sum, off));
         if (lane == 0u) a.partial[out * (zu64)NC + (zu64)j] = sum;
     }
+    if (SQ) {
+#pragma unroll
+        for (int j = 0; j < (SQ ? NC : 1); ++j) {
+            double sq = accq[j];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) sq = __dadd_rn(sq, __shfl_down_sync(0xFFFFFFFFu, sq, off));
+            if (lane == 0u) a.partial_q[out * (zu64)NC + (zu64)j] = sq;
+        }
+    }
 }
 
 /* One (cell, trial, chunk) unit: the warp's lanes stride over the chunk's sample groups [gb, ge), lane 0 takes the ragged tail,
@@ -893,7 +914,7 @@ template <class F, bool SQ>
 __device__ __forceinline__ void zmc_unit(const ZmcSampleArgs& a, const F& f, const ZmcKeySchedule& ks, const ZmcUnitCounter& uc,
                                          zu32 lane, zu32 gb, zu32 ge, zu32 gfe, zu32 full_groups, zu32 tail, zu64 out) {
     constexpr int D = F::D, SG = ZmcGroup<D>::SG, CG = ZmcGroup<D>::CG;
-    if constexpr (F::VEC) { zmc_unit_vec<F>(a, f, ks, uc, lane, gb, ge, gfe, full_groups, tail, out); return; }
+    if constexpr (F::VEC) { zmc_unit_vec<F, SQ>(a, f, ks, uc, lane, gb, ge, gfe, full_groups, tail, out); return; }
     /* acc[0..SG) sums the groups at even multiples of 32 from the lane's first one, acc[SG..2SG) those at odd multiples --
      * whatever UNROLL is, so results do not depend on it */
     double acc[2 * SG], accq[4];     /* sums of squares: two accumulators per group in flight are enough */

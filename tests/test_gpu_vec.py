@@ -12,7 +12,7 @@ from tests import vec_sources as VS
 pytestmark = pytest.mark.gpu
 
 
-def _make(dim, lower, upper, g, n, T, depth, m, seed, src, fn, C, precision, params=None, n_instances=1, budget=0, cap=1 << 16, **opts):
+def _make(dim, lower, upper, g, n, T, depth, m, seed, src, fn, C, precision, params=None, n_instances=1, budget=0, cap=1 << 16, opts=None):
     it = B.Integrator(dim, lower, upper, g, n, T, depth, m, seed)
     it.set_option(B.OPT_PRECISION, B.F32 if precision == O.F32 else B.F64)
     it.set_integrand_source_vec(src, fn, C, params, n_instances)
@@ -20,7 +20,7 @@ def _make(dim, lower, upper, g, n, T, depth, m, seed, src, fn, C, precision, par
     it.set_option(B.OPT_MAX_CELLS_PER_LEVEL, cap)
     if budget:
         it.set_option(B.OPT_MAX_GROUPS_PER_LEVEL, budget)
-    for k, v in opts.items():
+    for k, v in (opts or {}).items():
         it.set_option(k, v)
     cfg = O.Config(dim=dim, lower=lower, upper=upper, g=g, n_samples=n, trials=T, depth=depth, sigma_multiplier=m, seed=seed,
                    integrand=O.CONST, precision=precision, params=params, n_instances=n_instances, max_groups_per_level=budget)
@@ -197,6 +197,27 @@ def test_moments8_6d_sampled_units_and_full_control():
     it.close()
 
 
+@pytest.mark.parametrize("precision", [O.F32, O.F64])
+def test_spread_from_samples_per_component(precision):
+    """R13 + R15: sums of f_j^2 next to the sums of f_j, the spread of every component from its samples; whole tree against the oracle."""
+    it, cfg = _make(3, [0, 0, -1], [1, 2, 1], 3, 1003, 4, 3, 0.5, 5, VS.POLY4, "poly4", 4, precision, budget=3,
+                    opts={B.OPT_SPREAD: B.SPREAD_SAMPLES})
+    cfg.spread = O.SPREAD_SAMPLES
+    it.run()
+    ores = O.run_vec(cfg, 4, O.compile_user_fn(VS.POLY4, "poly4"), keep_cells=True)
+    assert len(ores.levels) == 3 and ores.levels[0].n_refined > 0
+    _compare(it, ores, 1003, scale=4.0)
+    for lev, ol in enumerate(ores.levels, start=1):
+        Q = it.level_sumsq(lev, ol.n_cells)
+        assert Q.shape == ol.Q.shape
+        assert np.abs(Q - ol.Q).max() <= 1e-12 * 1003 * 16.0
+    v, s = it.result()
+    closed = np.array([2.0, 4.0 / 3.0, 12.0, 2.0])
+    assert np.all(np.abs(v[0] - closed) <= 4.5 * s[0] + 1e-12)      # std is a 1-sigma error here
+    assert s[0, 2] == 0.0                                            # the constant component
+    it.close()
+
+
 def test_error_states():
     it = B.Integrator(2, [0, 0], [1, 1], 3, 100, 3, 2, 1.0, 1)
     with pytest.raises(B.ZmcError) as e:
@@ -205,16 +226,16 @@ def test_error_states():
     with pytest.raises(B.ZmcError) as e:
         it.set_integrand_source_vec(VS.TWO_AXES, "two_axes", 0)
     assert e.value.status == B.ERR_RANGE
-    it.set_option(B.OPT_SPREAD, B.SPREAD_SAMPLES)
+    it.set_option(B.OPT_BUDGET_ORDER, B.BUDGET_LARGEST_SPREAD)
     with pytest.raises(B.ZmcError) as e:
         it.set_integrand_source_vec(VS.TWO_AXES, "two_axes", 2)
     assert e.value.status == B.ERR_STATE
-    it.set_option(B.OPT_SPREAD, B.SPREAD_TRIALS)
+    it.set_integrand_source_vec(VS.AXIS0, "axis0", 1)              # one component: a largest-spread budget is defined
+    it.set_option(B.OPT_BUDGET_ORDER, B.BUDGET_PATH_ORDER)
     it.set_integrand_source_vec(VS.TWO_AXES, "two_axes", 2)
-    for key, val in ((B.OPT_SPREAD, B.SPREAD_SAMPLES), (B.OPT_BUDGET_ORDER, B.BUDGET_LARGEST_SPREAD)):
-        with pytest.raises(B.ZmcError) as e:
-            it.set_option(key, val)
-        assert e.value.status == B.ERR_STATE
+    with pytest.raises(B.ZmcError) as e:
+        it.set_option(B.OPT_BUDGET_ORDER, B.BUDGET_LARGEST_SPREAD)
+    assert e.value.status == B.ERR_STATE
     it.run()                                    # the context is still usable after the refusals
     v, s = it.result()
     assert v.shape == (1, 2) and np.all(np.isfinite(v)) and np.all(s > 0)
