@@ -166,6 +166,73 @@ __global__ void zmc_init_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_init
 
 /* R5: S_t = sum of the chunk partials in chunk order ; I_t = ((V*A)*S_t)/(double)N ;
  * mu = (sum_t I_t)/T ; s = sqrt((sum_t (I_t-mu)^2)/T)  -- two-pass, population form. */
+/* the (cell, component) entries first, first + step, .. < last: one thread per entry */
+__device__ __forceinline__ void zmc_cell_stats_span(const ZmcCtlArgs& c, const zu64 first, const zu64 last, const zu64 step) {
+    const ZmcLevelInfo& li = c.info[c.level];
+    const zu32 nch = li.n_chunks;
+    const double dN = (double)c.N, dT = (double)c.T;
+    zu64 bad = 0;
+    const zu64 nc = c.nc;
+    /* one thread per (cell, component): component j of work item i is partial[i * nc + j] (R15); nc == 1: one thread per cell */
+    for (zu64 e = first; e < last; e += step) {
+        const zu64 cell = (nc == 1ull) ? e : e / nc;
+        const zu64 jc = e - cell * nc;
+        double A = 1.0;
+        if (c.prefactor_index >= 0) {
+            const zu32 inst = c.cur.inst[cell / c.k];
+            A = c.params[(zu64)inst * (zu64)c.ppi + (zu64)c.prefactor_index];
+        }
+        const double VA = __dmul_rn(c.V, A);
+        const double* p = c.partial + cell * (zu64)c.T * nch * nc + jc;
+        /* the cell's T * n_chunks partial sums are read one after the other below (a dependent chain of FP64 adds): ask for their
+         * cache lines first, all at once, so that the chain does not pay an L2 round trip per trial */
+        if (nch > 1u || c.T > 4u) {
+            const char* q0 = (const char*)p;
+            const zu64 bytes = (zu64)c.T * nch * nc * sizeof(double);
+            for (zu64 off = 0; off < bytes; off += 128ull) asm volatile("prefetch.global.L1 [%0];" ::"l"(q0 + off));
+        }
+        double acc = 0.0;
+        for (zu32 t = 0; t < c.T; ++t) {
+            double S = p[(zu64)t * nch * nc];
+            for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]);
+            if (c.S) c.S[(cell * c.T + t) * nc + jc] = S;
+            acc = __dadd_rn(acc, __ddiv_rn(__dmul_rn(VA, S), dN));
+        }
+        const double mu = __ddiv_rn(acc, dT);
+        double sd;
+        if (c.spread == 0) {
+            double q = 0.0;
+            for (zu32 t = 0; t < c.T; ++t) {
+                double S = p[(zu64)t * nch * nc];
+                for (zu32 ch = 1; ch < nch; ++ch) S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]);
+                const double d = __dadd_rn(__ddiv_rn(__dmul_rn(VA, S), dN), -mu);
+                q = __dadd_rn(q, __dmul_rn(d, d));
+            }
+            sd = __dsqrt_rn(__ddiv_rn(q, dT));
+        } else {
+            /* R13: Sc = sum_t S_t, Qc = sum_t Q_t over M = T*N samples ; d = Qc - Sc^2/M, 0 unless d > Qc*2^-40 ;
+             * s = (V*A) * sqrt((d/M)/M), the standard error of mu. per component (R15) */
+            const double* pq = c.partial_q + cell * (zu64)c.T * nch * nc + jc;
+            double Sc = 0.0, Qc = 0.0;
+            for (zu32 t = 0; t < c.T; ++t) {
+                double S = p[(zu64)t * nch * nc], Q = pq[(zu64)t * nch * nc];
+                for (zu32 ch = 1; ch < nch; ++ch) { S = __dadd_rn(S, p[((zu64)t * nch + ch) * nc]); Q = __dadd_rn(Q, pq[((zu64)t * nch + ch) * nc]); }
+                if (c.Q) c.Q[(cell * c.T + t) * nc + jc] = Q;
+                Sc = __dadd_rn(Sc, S);
+                Qc = __dadd_rn(Qc, Q);
+            }
+            const double M = __dmul_rn(dT, dN);
+            double d = __dadd_rn(Qc, -__ddiv_rn(__dmul_rn(Sc, Sc), M));
+            if (!(d > __dmul_rn(Qc, 9.094947017729282e-13))) d = 0.0;
+            sd = __dmul_rn(VA, __dsqrt_rn(__ddiv_rn(__ddiv_rn(d, M), M)));
+        }
+        c.mu[e] = mu;
+        c.s[e] = sd;
+        if (!(fabs(mu) <= 1.7976931348623157e308) || !(fabs(sd) <= 1.7976931348623157e308)) ++bad;
+    }
+    if (bad) atomicAdd(c.nonfinite, bad);
+}
+
 /* One block, batches of floor(256 / T) entries (an entry = a (cell, component)); entries [e_begin, e_end), batches b_first, b_first + b_step, ..
  * One thread per (entry, trial) sums that trial's chunk partials (in chunk order) and forms I_t -- T independent loads and divisions side by side
  * instead of one thread walking them as a chain; then the entry's first thread adds the T values in trial order. The arithmetic of every number is what
@@ -244,9 +311,13 @@ __device__ __forceinline__ void zmc_cell_stats_batches(const ZmcCtlArgs& c, cons
     }
     if (bad) atomicAdd(c.nonfinite, bad);
 }
+/* Small levels (where the statistics are latency, not throughput) go one thread per (entry, trial); large ones one thread per entry, every
+ * thread busy -- the 4.5e8-cell level of BASELINE.json configs[1] whole: 18 ms against 34 ms. The numbers are the same bit for bit. */
 __device__ __forceinline__ void zmc_cell_stats_kernel_body(const ZmcCtlArgs& c, const zu32 bid, const zu32 nb) {
     __shared__ double sh[3 * ZMC_CTL_THREADS];
-    zmc_cell_stats_batches(c, 0ull, c.info[c.level].n_cells * (zu64)c.nc, bid, nb, sh);
+    const zu64 n_entries = c.info[c.level].n_cells * (zu64)c.nc;
+    if (n_entries <= (1ull << 18)) zmc_cell_stats_batches(c, 0ull, n_entries, bid, nb, sh);
+    else zmc_cell_stats_span(c, (zu64)bid * blockDim.x + threadIdx.x, n_entries, (zu64)nb * blockDim.x);
 }
 #ifndef ZMC_CONTROL_BODIES_ONLY
 __global__ void __launch_bounds__(ZMC_CTL_THREADS) zmc_cell_stats_kernel(const __grid_constant__ ZmcCtlArgs c) { zmc_cell_stats_kernel_body(c, blockIdx.x, gridDim.x); }
