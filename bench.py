@@ -73,6 +73,10 @@ DEVIATIONS = {
 }
 
 
+# total times the paper prints for its own parameter sets on one Tesla V100: context, not a target
+PAPER_SECONDS = {"paper_t3_sin6d": 38.7, "paper_t4_gauss9d": 4.8, "cfg12_gauss12d": 47.6}
+
+
 def capacity_for(w):
     """max_cells_per_level the bench (and the full-size parity tests) run a workload with: what its budget
     or depth bounds, else 0 = the library's automatic capacity."""
@@ -433,7 +437,10 @@ def main():
             line["time_to_result"] = {args.workload: {"ms": ms_per_step, "value": float(value_v[0]), "std": float(value_s[0])}}
             extra = ["cfg3_gauss9d",            # configs[2] whole, the paper's rule
                      "cfg2_sin6d_depth2",       # configs[1] under the paper's rule (no budget), levels 1-2 of 3 (~2.4 s)
-                     "cfg5_sin6d_depth4_B1"]    # configs[4] to depth 4 with one refined cell per level (~8 s)
+                     "cfg5_sin6d_depth4_B1",    # configs[4] to depth 4 with one refined cell per level (~8 s)
+                     "paper_t3_sin6d",          # the paper's own parameter sets (context: 38.7 s, 4.8 s and 47.6 s on one V100,
+                     "paper_t4_gauss9d",        #  other hardware, other stack)
+                     "cfg12_gauss12d"]
             for name in extra:
                 if name == args.workload:
                     continue
@@ -451,6 +458,8 @@ def main():
                     "flagged_per_level": [int(stx.level[l].n_flagged) for l in range(stx.levels)],
                     "refined_per_level": [int(stx.level[l].n_refined) for l in range(stx.levels)],
                     "deviation": DEVIATIONS.get(name)}
+                if name in PAPER_SECONDS:
+                    line["time_to_result"][name]["paper_seconds_on_one_V100"] = PAPER_SECONDS[name]
                 itx.close()
             # BASELINE.json configs[0] is launch-bound (microseconds of arithmetic): kernel by kernel vs one CUDA graph
             w1 = wl["cfg1_sin3d_f64"]
