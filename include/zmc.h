@@ -72,7 +72,8 @@ enum {
                                          BASELINE.json configs[0]); per-level times in zmc_stats are then 0 (default 0) */
     ZMC_OPT_SPREAD = 9,               /* ZMC_SPREAD_TRIALS (default, the paper: s = std of the T trial estimates) or
                                          ZMC_SPREAD_SAMPLES (R13: s = standard error of the cell mean from sum f and
-                                         sum f^2 of its T*N samples; zmc_result's std is then a 1-sigma error) */
+                                         sum f^2 of its T*N samples; zmc_result's std is then a 1-sigma error; per component for a
+                                         vector-valued integrand) */
     ZMC_OPT_BUDGET_ORDER = 10,        /* which flagged cells the budget keeps: ZMC_BUDGET_PATH_ORDER (default, R12) or
                                          ZMC_BUDGET_LARGEST_SPREAD (R14: the B largest s, equal ones in path order) */
     ZMC_OPT_SINGLE_LAUNCH = 11        /* the whole tree search as ONE cooperative kernel launch (grid-wide barriers between the
@@ -80,7 +81,9 @@ enum {
                                          launch-bound problems (BASELINE.json configs[0]; PAPER.md:162-184 is about this per-call
                                          overhead). Same device functions, bit-identical results. 0 never, 1 whenever the kernel
                                          exists (pre-compiled integrands, ZMC_SPREAD_TRIALS, path-order budget), 2 = auto (default):
-                                         when level 1 has at most 4e6 evaluations. zmc_stats: kernel_launches 1, per-level times 0 */
+                                         when level 1 has at most 4e6 evaluations. zmc_stats: kernel_launches 1; the per-level times come
+                                         from %globaltimer stamps at the kernel's grid barriers (ZMC_TREE_MARKS=1 in the environment prints
+                                         the finer split to stderr) */
 };
 enum { ZMC_F64 = 0, ZMC_F32 = 1 };
 enum { ZMC_MATH_EXACT = 0, ZMC_MATH_FAST = 1 };

@@ -6,14 +6,18 @@
  *   zmc_init_kernel        root parents, zeroed results, level-1 plan
  *   zmc_cell_stats_kernel  per-(cell,trial) partial sums -> S_t -> I_t -> (mu_c, s_c)          (R5; R13 from sum f^2)
  *   zmc_threshold_kernel   per sibling group: tau = mean(s) + m*pstd(s), number of s > tau      (R6)
+ *   zmc_threshold_pass_kernel<0,1,2>   the same for groups of several 4096-cell tiles, one launch per pass
  *   zmc_scan_kernel        exclusive scans over groups and instances -> output slots, next plan (R7, R12)
- *   zmc_select_kernel, zmc_count2_kernel, zmc_scan2_kernel
+ *   zmc_select_kernel (or, for few large instances, zmc_select_begin/hist/pick_kernel), zmc_count2_kernel, zmc_scan2_kernel
  *                          only with ZMC_BUDGET_LARGEST_SPREAD: radix select of the B largest flagged
  *                          spreads per instance, counts above / at the pivot, their scans            (R14)
  *   zmc_scatter_kernel     stable compaction of flagged cells into the next parent list;
  *                          accepted cells -> per-group (sum mu, sum s^2)                         (R7)
  *   zmc_accumulate_kernel  per instance: value += sum mu, var += sum s^2                         (R7)
  *   zmc_finalize_kernel    (value, sqrt(var)) per instance
+ *
+ * Every kernel is a device function (zmc_*_body) plus a one-line __global__ wrapper: the single-launch tree kernel (zmc_tree.cuh)
+ * calls the same bodies between grid barriers, and zmc_group_control_body fuses statistics, threshold and count for one group.
  *
  * Every reduction has a fixed shape (strided partials, then a tree), so repeated runs are
  * bit-identical. Nothing here is read by the host until zmc_result.

@@ -35,8 +35,7 @@ struct ZmcTreeArgs {
     double* result;
 };
 
-/* two 256-thread blocks per SM (128 registers) keep as many warps on the sampling phase as the multi-launch kernel has; FP64 at
- * high D would spill there */
+/* block 0 stamps %globaltimer as it passes the level's grid barriers: zmc_stats turns the stamps into per-level times */
 __device__ __forceinline__ void zmc_tree_mark(const ZmcCtlArgs& ca, zu32 level, int which) {
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         zu64 t;
@@ -45,6 +44,8 @@ __device__ __forceinline__ void zmc_tree_mark(const ZmcCtlArgs& ca, zu32 level, 
     }
 }
 
+/* two 256-thread blocks per SM (128 registers) keep as many warps on the sampling phase as the multi-launch kernel has; FP64 at
+ * high D would spill there */
 template <class F> struct ZmcTreeTune { static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && F::D >= 7) ? 1 : 2; };
 
 template <class F>
