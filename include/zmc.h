@@ -80,7 +80,7 @@ enum {
                                          sampling and control phases of every level) instead of 2 + 6*depth launches: for
                                          launch-bound problems (BASELINE.json configs[0]; PAPER.md:162-184 is about this per-call
                                          overhead). Same device functions, bit-identical results. 0 never, 1 whenever the kernel
-                                         exists (pre-compiled integrands, ZMC_SPREAD_TRIALS, path-order budget), 2 = auto (default):
+                                         exists (built-in integrands of at most 8 dimensions in FP64 or exact FP32, ZMC_SPREAD_TRIALS, path-order budget), 2 = auto (default):
                                          when level 1 has at most 4e6 evaluations. zmc_stats: kernel_launches 1; the per-level times come
                                          from %globaltimer stamps at the kernel's grid barriers (ZMC_TREE_MARKS=1 in the environment prints
                                          the finer split to stderr) */

@@ -16,7 +16,9 @@ static ZmcKernelEntry zmc_entry() {
     e.sample = (const void*)zmc_sample_kernel<F, false>;
     e.sample_ukey = (const void*)zmc_sample_kernel<F, true>;
     e.points = (const void*)zmc_points_kernel<F>;
-    e.tree = (const void*)zmc_tree_kernel<F>;
+    /* the single-launch tree kernel is for launch-bound problems: low dimensions, exact math (it doubles the compile time of an instance) */
+    if constexpr (D <= ZMC_TREE_MAX_DIM && ZMC_INST_MODE == ZMC_MODE_EXACT) e.tree = (const void*)zmc_tree_kernel<F>;
+    else e.tree = nullptr;
     return e;
 }
 

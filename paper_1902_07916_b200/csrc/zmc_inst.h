@@ -4,12 +4,13 @@
 #define ZMC_INST_H
 
 #define ZMC_AOT_MAX_DIM 12
+#define ZMC_TREE_MAX_DIM 8     /* zmc_tree_kernel<F> is pre-compiled for D <= 8, exact math */
 
 struct ZmcKernelEntry {
     const void* sample;       /* zmc_sample_kernel<F, false>: per-item key (batched instances) */
     const void* sample_ukey;  /* zmc_sample_kernel<F, true>: one key for the whole launch (n_instances == 1) */
     const void* points;   /* zmc_points_kernel<F> */
-    const void* tree;     /* zmc_tree_kernel<F>: the whole tree search as one cooperative launch (zmc_tree.cuh) */
+    const void* tree;     /* zmc_tree_kernel<F>: the whole tree search as one cooperative launch (zmc_tree.cuh); nullptr where not compiled */
 };
 
 #define ZMC_DECLARE_LOOKUP(PREC, MODE, ID) ZmcKernelEntry zmc_lookup_##PREC##_##MODE##_##ID(int dim);
