@@ -249,3 +249,46 @@ def test_error_states():
     v, s = it.result()
     assert v.shape == (1,)
     it.close()
+
+
+def test_bench_configuration_sampled_units_control_and_closed_forms():
+    """The vector-valued bench workload at its full size (bench.py `vector_valued`: 6-D, 4096 cells, N = 1e5, T = 5, 8 components):
+    sampled (cell, trial) units against the oracle, the control path re-derived in numpy, and all eight integrals against their
+    closed forms -- the raw moments of a sum of six uniforms, exact rationals."""
+    from fractions import Fraction
+    from math import comb
+    from paper_1902_07916_b200 import workloads as W
+    w = W.vec_moments6d()
+    C = 8
+    it = B.Integrator(w.dim, w.lower, w.upper, w.g, w.n_samples, w.trials, w.depth, w.sigma_multiplier, w.seed)
+    it.set_option(B.OPT_PRECISION, B.F32)
+    it.set_integrand_source_vec(W.VEC_MOMENTS_SRC, W.VEC_MOMENTS_FN, C, w.params, 1)
+    it.set_option(B.OPT_KEEP_LEVEL_STATS, 1)
+    it.set_option(B.OPT_MAX_CELLS_PER_LEVEL, w.k)
+    it.run()
+    v, s = it.result()
+    gl = it.level_cells(1)
+    assert len(gl.refined) == 4096 and gl.refined.sum() == 0            # depth 1: nothing refined
+    cfg = O.Config(dim=w.dim, lower=list(w.lower), upper=list(w.upper), g=w.g, n_samples=w.n_samples, trials=w.trials, depth=w.depth,
+                   sigma_multiplier=w.sigma_multiplier, seed=w.seed, integrand=O.CONST, precision=O.F32, params=w.params)
+    fns = O.compile_user_fn(W.VEC_MOMENTS_SRC, W.VEC_MOMENTS_FN)
+    rng = np.random.default_rng(11)
+    for cell in rng.integers(0, 4096, size=4):
+        path, coords = O.path_coords(6, 4, [int(cell)])
+        t = int(rng.integers(0, 5))
+        S = O.vec_unit_sums(cfg, C, fns, 0, path, 1, coords, t)
+        assert np.abs(gl.S[cell, t] - S).max() <= 1e-12 * w.n_samples * max(1.0, float(np.abs(S).max()) / w.n_samples)
+    V = (1.0 / 4) ** 6
+    I = gl.S * V / w.n_samples
+    mu = I.mean(axis=1)
+    np.testing.assert_allclose(gl.mu, mu, rtol=1e-12)
+    np.testing.assert_allclose(v[0], gl.mu.sum(axis=0), rtol=1e-12)
+    np.testing.assert_allclose(s[0], np.sqrt((gl.s ** 2).sum(axis=0)), rtol=1e-10)
+    # E[(x1 + .. + x6)^j] for independent uniforms: M_n(j) = sum_m C(j, m) M_{n-1}(j - m) / (m + 1)
+    M = [Fraction(1)] + [Fraction(0)] * C
+    for _ in range(6):
+        M = [sum(Fraction(comb(j, m)) * M[j - m] / (m + 1) for m in range(j + 1)) for j in range(C + 1)]
+    closed = np.array([float(Fraction(3, 10) ** j * M[j]) for j in range(1, C + 1)])
+    z = (v[0] - closed) / s[0]
+    assert np.all(np.abs(z) < 4.0), z
+    it.close()
