@@ -71,7 +71,7 @@ def _sources():
 def _stamp() -> str:
     h = hashlib.sha256()
     for name in sorted(os.listdir(CSRC)):
-        if name.endswith((".cu", ".cuh", ".h")) and name != "zmc_microbench.cu":
+        if name.endswith((".cu", ".cuh", ".h")) and name not in ("zmc_microbench.cu", "zmc_kernel_probe.cu"):
             h.update(name.encode())
             h.update(open(os.path.join(CSRC, name), "rb").read())
     h.update(open(os.path.join(os.path.dirname(HERE), "include", "zmc.h"), "rb").read())

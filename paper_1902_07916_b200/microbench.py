@@ -2,6 +2,10 @@
 library libzmc_microbench.so by build.build_microbench(); a measurement tool, not part of the product ABI).
 
     python -m paper_1902_07916_b200.microbench            # prints a markdown table (needs a B200)
+    python -m paper_1902_07916_b200.microbench --probe DIM INTEGRAND UKEY [-DNAME=VALUE ...] [-- n_inst g N T reps]
+        # one level-1 launch of the sampling kernel instance (csrc/zmc_kernel_probe.cu, compiled on the spot with the given
+        # macros): evaluations/s, fraction of the ALU roof, checksum. E.g. the per-item-key cost at D = 4:
+        #   --probe 4 3 0 -- 256 6 4096 5 4      against      --probe 4 3 1 -- 256 6 4096 5 4
 
 They give the denominator of the ALU roofline: warp-instructions per SM per clock
 for IMAD.WIDE.U32, LOP3, FFMA, ... and whole Philox4x32-10 calls.
@@ -70,6 +74,35 @@ def mix_table():
         print("| %s | " % MIX[x] + " | ".join("%.1f" % c for c in clk) + " | %.2f |" % ((clk[-1] - clk[0]) / MIX_K[-1]))
 
 
+def probe(argv):
+    """Compile csrc/zmc_kernel_probe.cu for one kernel instance (nvcc, sm_100a, the product's flags) and run it."""
+    import os
+    import subprocess
+    import tempfile
+    run_args = []
+    if "--" in argv:
+        i = argv.index("--")
+        argv, run_args = argv[:i], argv[i + 1:]
+    dim, integrand, ukey = argv[0], argv[1], argv[2]
+    defs = ["-DTD=%s" % dim, "-DTID=%s" % integrand, "-DTUKEY=%s" % ukey] + list(argv[3:])
+    exe = os.path.join(tempfile.gettempdir(), "zmc_kernel_probe_%d" % os.getpid())
+    cmd = [_build.NVCC, *_build.ARCH, "-O3", "-std=c++17", "--fmad=false", "-lineinfo", "-diag-suppress", "550", "-Xptxas", "-v",
+           *defs, "-I", _build.CSRC, os.path.join(_build.CSRC, "zmc_kernel_probe.cu"), "-o", exe]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(cmd), r.stderr[-4000:]))
+    regs = [ln.strip() for ln in r.stderr.splitlines() if "registers" in ln]
+    print(" ".join(defs), "|", regs[0] if regs else "", flush=True)
+    try:
+        subprocess.run([exe, *run_args], check=True)
+    finally:
+        os.unlink(exe)
+
+
 if __name__ == "__main__":
-    main()
-    mix_table()
+    import sys
+    if len(sys.argv) > 1 and sys.argv[1] == "--probe":
+        probe(sys.argv[2:])
+    else:
+        main()
+        mix_table()
