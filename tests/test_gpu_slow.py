@@ -151,3 +151,34 @@ def test_config2_whole_under_the_papers_rule():
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     json.dump(out, open(os.path.join(ROOT, "gpurun_out", "r2_cfg2_whole.json"), "w"), indent=1)
     it.close()
+
+
+@pytest.mark.skipif(os.environ.get("ZMC_RUN_SLOW") != "1", reason="~7 minutes of the oracle on one host core; set ZMC_RUN_SLOW=1")
+def test_config3_whole_gpu_against_the_oracle_whole():
+    """BASELINE.json configs[2] WHOLE on both sides: the 9-D narrow Gaussian, 4 levels x 19 683 cells, 7.87e9 evaluations. The oracle
+    runs the complete tree on one host core (~6 minutes: its time-to-result, measured, not extrapolated) and every one of the 78 732
+    cells is compared -- per-(cell, trial) sums, (mu, s), tau, refined sets, cell identities -- plus the result. Run it alone:
+
+        ZMC_RUN_SLOW=1 python -m pytest tests/test_gpu_slow.py -m gpu -s -k config3
+    """
+    w = W.config3()
+    it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=w.max_cells_per_level)
+    it.run()
+    v, s = it.result()
+    st = it.stats()
+    t0 = time.perf_counter()
+    ores = O.run(H.oracle_config(w), keep_cells=True)
+    oracle_s = time.perf_counter() - t0
+    n = H.compare_tree(it, ores, w)
+    assert n == 4 * 19683
+    closed = H.closed_exp_quad(w.params[0], w.lower, w.upper)
+    assert abs(v[0] - closed) <= 4 * s[0]
+    rec = {"workload": "cfg3_gauss9d (BASELINE.json configs[2], whole)", "cells_compared": n, "value_gpu": float(v[0]), "std_gpu": float(s[0]),
+           "value_oracle": float(ores.value[0]), "std_oracle": float(ores.std[0]), "closed_form": closed,
+           "evals": int(st.total_evals), "gpu_device_ms": float(st.total_ms), "oracle_seconds_one_core": oracle_s,
+           "oracle_evals_per_s": st.total_evals / oracle_s, "refined_per_level": [int(st.level[l].n_refined) for l in range(4)]}
+    print(json.dumps(rec))
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "r2_cfg3_whole_vs_oracle.json"), "w") as f:
+        json.dump(rec, f, indent=1)
+    it.close()
