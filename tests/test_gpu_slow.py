@@ -13,6 +13,9 @@ Checked at that size (the oracle cannot run it whole):
   * all levels: sampled units against the oracle;
   * result within 4 sigma of the closed form; the z-score against std/sqrt(T-1) is printed.
 A JSON summary goes to gpurun_out/r2_cfg2_whole.json (profiles/r2_cfg2_whole.md quotes it).
+
+Second slow test: BASELINE.json configs[2] (9-D narrow Gaussian) whole on BOTH sides -- the oracle's complete tree on one host core
+(~9 minutes) against the GPU's, all 78 732 cells (-k config3).
 """
 import json
 import math
