@@ -232,6 +232,40 @@ int zmc_debug_words(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t 
 int zmc_debug_points(zmc_ctx* ctx, uint32_t instance, uint64_t path_lo, uint32_t path_hi, int level,
                      const uint32_t* coords, int trial, uint64_t n, double* x, double* f);
 
+/* ---- One level of stratified sampling WITHOUT any device-memory allocation ------------------------------------------------------
+ * For callers that cannot allocate on the GPU: a process whose device memory is already spoken for down to the last byte (another
+ * component's memory pool holds the card, so cudaMalloc fails), or a latency-critical loop that must not meet the device-wide
+ * synchronisation of cudaMalloc / cudaFree. zmc_run is closed to them -- it allocates its workspace, or needs one somebody allocated.
+ *
+ * zmc_flat_static computes what zmc_create(.., depth = 1, ..) + zmc_set_integrand + zmc_run + zmc_result compute for ONE instance of a
+ * built-in integrand (every cell of the g^D grid sampled `trials` times with `samples_per_cell` points; per-cell mean
+ * and spread; value = sum of the cell means, std = sqrt of the sum of the cell variances, R5, R7), with the same device
+ * functions and therefore the same bits. All of its scratch memory is a fixed array inside the library image:
+ *   - every GPU that loads the library's kernels holds ZMC_STATIC_SCRATCH_BYTES (2 MiB) for it until the process exits;
+ *   - the problem must fit: divisions_per_axis^dim <= ZMC_STATIC_MAX_CELLS, cells * trials <= ZMC_STATIC_MAX_UNITS, dim <= 12
+ *     (pre-compiled kernels only), n_params <= ZMC_STATIC_MAX_PARAMS; anything larger is refused with ZMC_ERR_CAPACITY (ZMC_ERR_RANGE
+ *     for dim) and a message that names the limit -- nothing is launched;
+ *   - ALL calls on one GPU share the array. Calls that follow one another on one stream are fine (each call resets what it needs and
+ *     never reads what an earlier call left). Calls that can overlap on the GPU -- different streams, or different host threads --
+ *     race on it and give garbage: serialise them.
+ * The call itself runs no cudaMalloc, cudaFree or other allocating routine, enqueues three kernels on cuda_stream and returns without
+ * synchronising. The FIRST call on each device also looks up the array's address on that device (cudaGetSymbolAddress, with the
+ * caller's current device) and the SM count, and makes the runtime load the kernels there; make that first call at start-up, before
+ * any stream capture, not in the middle of one.
+ *   dim, lower, upper, divisions_per_axis, samples_per_cell, trials, seed     as zmc_create ([host] arrays, read during the call)
+ *   builtin_id, params [host], n_params      as zmc_set_integrand with one instance (ZMC_USER is refused: NVRTC allocates)
+ *   precision, math    ZMC_F64 / ZMC_F32, ZMC_MATH_EXACT / ZMC_MATH_FAST (as the options of the same names)
+ *   result             [device] 2 doubles, caller-owned: value, std -- valid once the work enqueued on cuda_stream has finished
+ *   cuda_stream        a cudaStream_t (NULL = the default stream)
+ *   err, err_len       [host] optional buffer for the reason of a failure (NUL-terminated, "" on success); may be NULL / 0 */
+#define ZMC_STATIC_SCRATCH_BYTES (2u << 20)
+#define ZMC_STATIC_MAX_CELLS 4096
+#define ZMC_STATIC_MAX_UNITS 131072
+#define ZMC_STATIC_MAX_PARAMS 32
+int zmc_flat_static(int dim, const double* lower, const double* upper, int divisions_per_axis, uint64_t samples_per_cell, int trials,
+                    uint64_t seed, int builtin_id, const double* params, int n_params, int precision, int math, double* result,
+                    void* cuda_stream, char* err, size_t err_len);
+
 /* The reason of the last failure on ctx ("" if none; valid until the next call on ctx). ctx == NULL: the reason of the calling
  * thread's last failed zmc_create (valid until that thread's next zmc_create). */
 const char* zmc_last_error(const zmc_ctx* ctx);

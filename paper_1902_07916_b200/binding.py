@@ -32,7 +32,8 @@ MAX_DEPTH = 15
 
 EXPORTS = ["zmc_create", "zmc_set_integrand", "zmc_set_integrand_source", "zmc_set_integrand_source_vec", "zmc_set_option", "zmc_workspace_bytes",
            "zmc_set_workspace", "zmc_run", "zmc_result", "zmc_stats", "zmc_level_cells", "zmc_level_cells_range", "zmc_level_sumsq", "zmc_debug_words",
-           "zmc_debug_points", "zmc_last_error", "zmc_status_string", "zmc_destroy"]
+           "zmc_debug_points", "zmc_flat_static", "zmc_last_error", "zmc_status_string", "zmc_destroy"]
+STATIC_SCRATCH_BYTES, STATIC_MAX_CELLS, STATIC_MAX_UNITS, STATIC_MAX_PARAMS = 2 << 20, 4096, 131072, 32
 
 _INTEGRAND_ID = {W.CONST: CONST, W.LINEAR: LINEAR, W.SIN_SUM: SIN_SUM, W.EXP_QUAD: EXP_QUAD}
 _PRECISION_ID = {W.F64: F64, W.F32: F32}
@@ -91,6 +92,8 @@ def lib():
     L.zmc_level_sumsq.argtypes = [vp, C.c_int, C.c_uint64, dp]
     L.zmc_debug_words.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_uint64, C.c_uint64, u32p]
     L.zmc_debug_points.argtypes = [vp, C.c_uint32, C.c_uint64, C.c_uint32, C.c_int, u32p, C.c_int, C.c_uint64, dp, dp]
+    L.zmc_flat_static.argtypes = [C.c_int, dp, dp, C.c_int, C.c_uint64, C.c_int, C.c_uint64, C.c_int, dp, C.c_int, C.c_int, C.c_int,
+                                  vp, vp, C.c_char_p, C.c_size_t]
     L.zmc_last_error.argtypes = [vp]
     L.zmc_last_error.restype = C.c_char_p
     L.zmc_status_string.argtypes = [C.c_int]
@@ -278,6 +281,27 @@ class Integrator:
         self._check(self._L.zmc_debug_points(self._h, instance, path & (2 ** 64 - 1), path >> 64, level,
                                              _ptr(cc, C.c_uint32), trial, n, _dp(x), _dp(f)))
         return x, f
+
+
+def flat_static(dim: int, lower: Sequence[float], upper: Sequence[float], divisions_per_axis: int, samples_per_cell: int, trials: int,
+                seed: int, builtin_id: int, params: Optional[np.ndarray], precision: int, math: int, result_device_ptr: int,
+                stream: Optional[int] = None) -> None:
+    """zmc_flat_static: one level of stratified sampling whose scratch memory is a fixed array inside libzmc.so -- the call for hosts
+    that cannot allocate device memory (the card is owned by somebody else's pool, or cudaMalloc's synchronisation is not acceptable).
+    `result_device_ptr` is the address of 2 doubles in device memory that the caller owns (value, std); they are valid once `stream`
+    has finished. Nothing is allocated and nothing is synchronised here; calls that overlap on the GPU share the scratch and race."""
+    L = lib()
+    lo = np.ascontiguousarray(lower, dtype=np.float64)
+    up = np.ascontiguousarray(upper, dtype=np.float64)
+    p = None if params is None else np.ascontiguousarray(params, dtype=np.float64).reshape(-1)
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    err = C.create_string_buffer(512)
+    rc = L.zmc_flat_static(dim, _dp(lo), _dp(up), divisions_per_axis, samples_per_cell, trials, seed, builtin_id, _dp(p),
+                           0 if p is None else p.size, precision, math, C.c_void_p(result_device_ptr), C.c_void_p(stream), err, len(err))
+    if rc != OK:
+        raise ZmcError(rc, err.value.decode())
 
 
 def from_workload(w: W.Workload, math: int = MATH_EXACT, keep_level_stats: bool = False,

@@ -5,7 +5,7 @@
 Steps
   1. csrc/zmc_device.cuh -> csrc/zmc_device_src.inc (the same text as a C++ raw string literal,
      handed to NVRTC at run time for user integrands and for 12 < D <= 16);
-  2. nvcc -c, in parallel: zmc_lib.cu and zmc_inst.cu once per pre-compiled
+  2. nvcc -c, in parallel: zmc_lib.cu, zmc_static.cu and zmc_inst.cu once per pre-compiled
      (precision, math mode, integrand) combination;
   3. nvcc -shared -cudart static -> paper_1902_07916_b200/libzmc.so.
 build_microbench() makes the pipe-rate probes of csrc/zmc_microbench.cu a library of their own
@@ -61,7 +61,8 @@ def _write_source_inc() -> str:
 
 
 def _sources():
-    jobs = [("zmc_lib", os.path.join(CSRC, "zmc_lib.cu"), [])]
+    jobs = [("zmc_lib", os.path.join(CSRC, "zmc_lib.cu"), []),
+            ("zmc_static", os.path.join(CSRC, "zmc_static.cu"), [])]      # zmc_flat_static: the entry point that allocates nothing
     for p, m, i in COMBOS:
         jobs.append(("zmc_inst_%d_%d_%d" % (p, m, i), os.path.join(CSRC, "zmc_inst.cu"),
                      ["-DZMC_INST_PREC=%d" % p, "-DZMC_INST_MODE=%d" % m, "-DZMC_INST_ID=%d" % i]))
