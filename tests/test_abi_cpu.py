@@ -127,13 +127,18 @@ def test_binding_constants_match_the_header():
         "ZMC_OPT_PRECISION": B.OPT_PRECISION, "ZMC_OPT_MATH": B.OPT_MATH, "ZMC_OPT_MAX_GROUPS_PER_LEVEL": B.OPT_MAX_GROUPS_PER_LEVEL,
         "ZMC_OPT_KEEP_LEVEL_STATS": B.OPT_KEEP_LEVEL_STATS, "ZMC_OPT_MAX_CELLS_PER_LEVEL": B.OPT_MAX_CELLS_PER_LEVEL,
         "ZMC_OPT_GRID_BLOCKS": B.OPT_GRID_BLOCKS, "ZMC_OPT_TARGET_ITEMS": B.OPT_TARGET_ITEMS, "ZMC_OPT_USE_GRAPH": B.OPT_USE_GRAPH,
-        "ZMC_OPT_SPREAD": B.OPT_SPREAD, "ZMC_OPT_BUDGET_ORDER": B.OPT_BUDGET_ORDER,
+        "ZMC_OPT_SPREAD": B.OPT_SPREAD, "ZMC_OPT_BUDGET_ORDER": B.OPT_BUDGET_ORDER, "ZMC_OPT_SINGLE_LAUNCH": B.OPT_SINGLE_LAUNCH,
         "ZMC_F64": B.F64, "ZMC_F32": B.F32, "ZMC_MATH_EXACT": B.MATH_EXACT, "ZMC_MATH_FAST": B.MATH_FAST,
         "ZMC_SPREAD_TRIALS": B.SPREAD_TRIALS, "ZMC_SPREAD_SAMPLES": B.SPREAD_SAMPLES,
         "ZMC_BUDGET_PATH_ORDER": B.BUDGET_PATH_ORDER, "ZMC_BUDGET_LARGEST_SPREAD": B.BUDGET_LARGEST_SPREAD,
     }
     for name, value in mirror.items():
         assert enums[name] == value, name
+    # the fixed limits of zmc_flat_static are #defines
+    defs = dict(re.findall(r"#define\s+(ZMC_STATIC_[A-Z_]+)\s+(.+)", text))
+    assert eval(defs["ZMC_STATIC_SCRATCH_BYTES"].replace("u", "")) == B.STATIC_SCRATCH_BYTES
+    assert int(defs["ZMC_STATIC_MAX_CELLS"]) == B.STATIC_MAX_CELLS and int(defs["ZMC_STATIC_MAX_UNITS"]) == B.STATIC_MAX_UNITS
+    assert int(defs["ZMC_STATIC_MAX_PARAMS"]) == B.STATIC_MAX_PARAMS
     assert int(re.search(r"#define ZMC_MAX_DEPTH (\d+)", text).group(1)) == B.MAX_DEPTH
     # struct sizes as the C compiler sees them
     src = '#include <stdio.h>\n#include "zmc.h"\nint main(void) { printf("%zu %zu\\n", sizeof(zmc_level_stats), sizeof(zmc_stats_t)); return 0; }\n'
