@@ -63,6 +63,22 @@ def test_largest_spread_budget_whole_trees(name, spread):
     it.close()
 
 
+def test_largest_spread_budget_with_many_instances():
+    """With 64 instances or more (kSelectWideBelow in zmc_lib.cu) the radix select of R14 is ONE kernel with one block per instance
+    (zmc_select_kernel) instead of the begin / histogram / pick launches over all tiles that every other R14 test takes (they have 1 to
+    6 instances). 70 batched 4-D Gaussians, a binding budget of 2 cells per instance and level, three levels, against the oracle:
+    pivot, quota and tile range of that kernel decide which cells are refined, so identical refined sets cover them."""
+    w = W.config4(n_instances=70).with_(n_samples=40, depth=3, sigma_multiplier=0.5, max_groups_per_level=2)
+    it, ores = _both(w, B.SPREAD_TRIALS, B.BUDGET_LARGEST_SPREAD)
+    H.compare_tree(it, ores, w)
+    st = it.stats()
+    assert st.level[0].n_flagged > st.level[0].n_refined == 2 * w.n_instances       # every instance has at least 2 flagged cells, most far more: the budget binds
+    assert st.level[1].n_flagged > st.level[1].n_refined == 2 * w.n_instances
+    byp = O.run(H.oracle_config(w), keep_cells=True)
+    assert any(not np.array_equal(a.refined, b.refined) for a, b in zip(ores.levels, byp.levels))   # and the order matters
+    it.close()
+
+
 def test_options_switch_kernels_and_layout():
     """Changing the spread after a run re-selects the kernel and re-lays the workspace; results match fresh contexts."""
     w = W.config1()
