@@ -81,7 +81,10 @@ enum {
                                          launch-bound problems (BASELINE.json configs[0]; PAPER.md:162-184 is about this per-call
                                          overhead). Same device functions, bit-identical results. 0 never, 1 whenever the kernel
                                          exists (built-in integrands of at most 8 dimensions in FP64 or exact FP32, ZMC_SPREAD_TRIALS, path-order budget), 2 = auto (default):
-                                         when level 1 has at most 4e6 evaluations. zmc_stats: kernel_launches 1; the per-level times come
+                                         when level 1 has at most 4e6 evaluations and no later level can have more than 6.4e7 (by the budget,
+                                         by depth 2, or by the level capacity). 1 and 2 are preferences: if the driver refuses the
+                                         cooperative launch (fewer SMs than the device reports under an MPS thread percentage or a green
+                                         context; a tool in between) the run goes kernel by kernel, with the same bits. zmc_stats: kernel_launches 1; the per-level times come
                                          from %globaltimer stamps at the kernel's grid barriers (ZMC_TREE_MARKS=1 in the environment prints
                                          the finer split to stderr) */
 };
