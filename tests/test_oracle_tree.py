@@ -279,3 +279,19 @@ def test_narrow_gaussian_tree_homes_in_fp32_extended_range():
     assert abs(r.value[0] - 1.0) < 4 * r.std[0] and r.std[0] < 0.05
     r64 = O.run(H.oracle_config(small, precision=O.F64))
     assert abs(r64.value[0] - 1.0) < 4 * r64.std[0]
+
+
+def test_fanned_out_driver_is_the_oracle_bit_for_bit():
+    """tests/whole_tree.oracle_tree_fanned (per-unit sums in a process pool, then orc_cell_stats / orc_threshold level by level) is what the
+    GPU suite uses for BASELINE.json configs[2] whole; here it is pinned to oracle.run on small trees: every number the same bits."""
+    from tests import whole_tree as WT
+    for w in (W.config1(), W.config3().with_(g=2, n_samples=40, depth=3, sigma_multiplier=0.5),
+              W.Workload("s2", 2, (0.0, 0.0), (7.0, 5.0), 5, 64, 5, 4, 0.3, 9, W.SIN_SUM, W.F32)):
+        a = O.run(H.oracle_config(w), keep_cells=True)
+        b = WT.oracle_tree_fanned(w, processes=2, cells_per_job=7)
+        assert len(a.levels) == len(b.levels) and a.evals == b.evals
+        for la, lb in zip(a.levels, b.levels):
+            assert (la.n_cells, la.n_refined) == (lb.n_cells, lb.n_refined) and la.path == lb.path
+            for f in ("instance", "S", "mu", "s", "tau", "refined"):
+                np.testing.assert_array_equal(getattr(la, f), getattr(lb, f), err_msg=f)
+        assert abs(a.value[0] - b.value[0]) <= 1e-13 * max(abs(a.value[0]), a.std[0]) and abs(a.std[0] - b.std[0]) <= 1e-13 * a.std[0]
