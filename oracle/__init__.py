@@ -344,17 +344,26 @@ def compile_user_fn(src: str, fn_name: str, precisions=("f64", "f32")):
         wrap.append('extern "C" void orc_user_entry_f32(const float* x, int dim, const float* p, int np, float* out, int n_out) '
                     "{ %s(x, dim, p, np, out, n_out); }\n" % fn_name)
     text = "".join(wrap)
-    d = os.path.join(tempfile.gettempdir(), "zmc_oracle_user")
-    os.makedirs(d, exist_ok=True)
+    # a directory of this user's own (0700, ownership and mode checked): a library found there was put there by this user, and nobody else
+    # can plant one under the predictable name; source and library are written under pid-unique names and renamed into place
+    d = os.path.join(tempfile.gettempdir(), "zmc_oracle_user_%d" % os.getuid())
+    os.makedirs(d, mode=0o700, exist_ok=True)
+    st = os.lstat(d)
+    import stat as _stat
+    if not _stat.S_ISDIR(st.st_mode) or st.st_uid != os.getuid() or (st.st_mode & 0o077):
+        raise RuntimeError("%s is not a directory owned by this user with mode 0700: refusing to load libraries from it" % d)
     tag = hashlib.sha256(text.encode()).hexdigest()[:24]
     so = os.path.join(d, "user_%s.so" % tag)
     if not os.path.exists(so):
-        cpp = os.path.join(d, "user_%s.cpp" % tag)
+        cpp = os.path.join(d, "user_%s.%d.cpp" % (tag, os.getpid()))
         with open(cpp, "w") as f:
             f.write(text)
         tmp = so + ".tmp%d" % os.getpid()
-        subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-mfma", "-fPIC", "-shared", "-o", tmp, cpp], check=True)
-        os.replace(tmp, so)
+        try:
+            subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-mfma", "-fPIC", "-shared", "-o", tmp, cpp], check=True)
+            os.replace(tmp, so)
+        finally:
+            os.remove(cpp)
     L = C.CDLL(so)
     f64 = C.cast(L.orc_user_entry_f64, USER_F64) if "f64" in precisions else None
     f32 = C.cast(L.orc_user_entry_f32, USER_F32) if "f32" in precisions else None
