@@ -63,7 +63,12 @@ enum {
     ZMC_OPT_MAX_GROUPS_PER_LEVEL = 3, /* refinement budget B per instance and level, first B flagged cells in path
                                          order (R12); 0 = off = the paper's semantics (default) */
     ZMC_OPT_KEEP_LEVEL_STATS = 4,     /* 1: keep every level's per-cell arrays for zmc_level_cells (default 0) */
-    ZMC_OPT_MAX_CELLS_PER_LEVEL = 5,  /* capacity of one level in cells; 0 = auto (default) */
+    ZMC_OPT_MAX_CELLS_PER_LEVEL = 5,  /* capacity of one level in cells. 0 = automatic (default): sized for the budget if there is one; else a
+                                         modest guess (128 x level 1, within 2^22 .. 2^28 cells), and if a level outgrows it the search stops
+                                         there, zmc_result learns what that level needed, allocates a workspace for it (library-owned
+                                         workspaces only, if the device has the memory) and runs the search again -- same seeds, same bits as
+                                         a run that had the room from the start. BASELINE.json configs[1] as given (4.5e8 cells at level 3)
+                                         runs this way with no option set. A value > 0 is a hard limit: ZMC_ERR_CAPACITY beyond it */
     ZMC_OPT_GRID_BLOCKS = 6,          /* persistent sampling grid in CTAs; 0 = auto (SM count x resident CTAs) */
     ZMC_OPT_TARGET_ITEMS = 7,         /* a level with fewer (cell,trial) units than this is split into sample chunks
                                          until it has about this many work items (default 65536) */
@@ -165,7 +170,9 @@ int zmc_run(zmc_ctx* ctx, void* cuda_stream);
 /* Synchronise the run's stream and fetch, per instance, the integral estimate (sum of accepted cell
  * means) and its standard deviation (sqrt of the sum of accepted cell variances, R7).
  * value, std [host] n_instances doubles each (n_instances * n_components, [instance][component], for a vector-valued
- * integrand). Returns ZMC_ERR_CAPACITY if a level overflowed. */
+ * integrand). If a level overflowed: with the automatic capacity and a library-owned workspace the workspace is grown to what
+ * that level needed and the search is run again from here, on the same stream, once per overflowing level (this call then takes
+ * as long as those runs); otherwise ZMC_ERR_CAPACITY, and zmc_last_error says which level needed how many cells. */
 int zmc_result(zmc_ctx* ctx, double* value, double* std);
 
 typedef struct zmc_level_stats {

@@ -95,6 +95,8 @@ struct ZmcCtlArgs {
     zu64* excl_eq;
     zu64* sel_state;        /* [instance][4] prefix, need, above, active: the radix select spread over the grid (few, large instances) */
     zu64* sel_hist;         /* [instance][256] */
+    zu32 stop_on_overflow;  /* 1: a level that does not fit ends the search (the next level is empty) instead of going on with the parents that fit --
+                               the host grows the workspace and runs again, so what would follow is wasted time */
 };
 
 /* plan of one level: how the (cell, trial) units are cut into work items. (Tried and not kept: choosing the number of chunks
@@ -571,7 +573,7 @@ __device__ __forceinline__ void zmc_scan_kernel_body(const ZmcCtlArgs& c) {
     }
     if (threadIdx.x == 0) {
         zu64 n_next = carry;
-        if (n_next > c.cap_par) { n_next = c.cap_par; *c.overflow = 1u; }
+        if (n_next > c.cap_par) { n_next = c.stop_on_overflow ? 0ull : c.cap_par; *c.overflow = 1u; }
         c.info[c.level].n_flagged = total_flagged;
         c.info[c.level].n_refined = n_next;
         ZmcLevelInfo li;

@@ -117,3 +117,38 @@ def test_work_items_beyond_2_32():
     print("items > 2^32: level 2 has %d cells = %.3e work items; %d units against the oracle; level-2 sampling %.1f ms, control %.1f ms" %
           (n2, n2 * T, n_units, st.level[1].sample_ms, st.level[1].control_ms))
     it.close()
+
+
+def test_automatic_capacity_grows_to_what_the_tree_needs():
+    """BASELINE.json configs[1] as given must run through zmc_create / zmc_set_integrand / zmc_run / zmc_result with NO option set. Its
+    level 3 has 4.5e8 cells, far beyond the first automatic guess (2^22): the search stops at the overflow, zmc_result reads what level 3
+    needed, re-allocates and runs again. Here on the N = 8 tree of the same shape (4.43e8 cells): same bits as a run that was given the
+    room up front, the level sizes of the kept-array test above, and a workspace sized to the need. A caller-owned workspace cannot
+    grow: ZMC_ERR_CAPACITY with the need in the message."""
+    import torch
+    torch.cuda.empty_cache()
+    w = W.config2(depth=3, budget=0).with_(n_samples=8)
+    it = B.from_workload(w)                                   # precision and math mode only
+    it.run()
+    v, s = it.result()                                        # grows and re-runs inside
+    st = it.stats()
+    assert st.overflow == 0
+    assert [st.level[l].n_cells for l in range(3)] == [4096, 306 * 4096, 108142 * 4096]
+    grown = it.workspace_bytes()
+    it.close()
+    assert grown < 32 * 2 ** 30                               # 4.43e8 * (1 + 1/16) cells, 56 bytes each
+    ref = B.from_workload(w, max_cells_per_level=108142 * 4096)
+    ref.run()
+    v0, s0 = ref.result()
+    ref.close()
+    np.testing.assert_array_equal(v, v0)
+    np.testing.assert_array_equal(s, s0)
+    # a workspace the caller owns is a hard limit
+    it = B.from_workload(w)
+    it.use_torch_workspace()
+    it.run()
+    with pytest.raises(B.ZmcError) as e:
+        it.result()
+    assert e.value.status == B.ERR_CAPACITY and "level 3 needed 442949632 cells" in str(e.value), str(e.value)
+    it.close()
+    torch.cuda.empty_cache()

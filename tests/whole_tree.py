@@ -84,11 +84,11 @@ def check_config2_shaped_tree(w: W.Workload, max_cells_per_level: int, seed: int
     assert L == 3 and w.max_groups_per_level == 0
     rng = np.random.default_rng(seed)
     it = B.from_workload(w, keep_level_stats=True, max_cells_per_level=max_cells_per_level)
-    ws_bytes = it.workspace_bytes()
     t0 = time.perf_counter()
     it.run()
-    v, sd = it.result()
+    v, sd = it.result()           # max_cells_per_level == 0: the automatic capacity grows here and the search runs again
     wall = time.perf_counter() - t0
+    ws_bytes = it.workspace_bytes()
     st = it.stats()
     assert st.overflow == 0 and st.nonfinite == 0
     lv = [st.level[l] for l in range(L)]
@@ -179,6 +179,6 @@ def check_config2_shaped_tree(w: W.Workload, max_cells_per_level: int, seed: int
            "evals": int(st.total_evals), "device_ms": float(st.total_ms), "wall_s_run_plus_result": wall,
            "evals_per_s": st.total_evals / (st.total_ms * 1e-3),
            "sample_ms_per_level": [float(x.sample_ms) for x in lv], "control_ms_per_level": [float(x.control_ms) for x in lv],
-           "workspace_bytes": int(ws_bytes), "max_cells_per_level": int(max_cells_per_level), "level3_groups_checked_in_full": n_checked_groups}
+           "workspace_bytes": int(ws_bytes), "max_cells_per_level": int(max_cells_per_level) or "automatic (grown by zmc_result)", "level3_groups_checked_in_full": n_checked_groups}
     it.close()
     return rec
