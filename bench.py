@@ -117,11 +117,37 @@ def fp32_ops_per_eval(w):
     return 2 * w.dim
 
 
+# FP64 instructions per evaluation of the built-in integrands in FP64 mode (R8; the op sequences of ZmcMapF64 / ZmcIntegrand<.., F64>):
+# map 3 per dimension (DADD for (double)w + 0.5, DMUL, DADD); SIN_SUM: D-1 DADD + 15 (zmc_zsin64); EXP_QUAD: 3D - 1 (quadratic form) + 1 +
+# ~20 (libdevice exp); 1 DADD into the per-lane sum. The FP64 pipe takes one warp-instruction per 2 clocks per scheduler (profiles/r1_microbench.md).
+FP64_CLK_PER_WARP_INST = 2.0
+
+
+def fp64_ops_per_eval(w):
+    if w.integrand == "sin_sum":
+        return 3 * w.dim + (w.dim - 1) + 15 + 1
+    if w.integrand == "exp_quad":
+        return 3 * w.dim + (3 * w.dim - 1) + 1 + 20 + 1
+    if w.integrand == "linear":
+        return 3 * w.dim + 2 * w.dim + 1
+    return 3 * w.dim + 1
+
+
+def fp64_peak_evals_per_s(w, n_sm, sm_mhz):
+    """FP64-pipe roof (C = max(4 n_imad, 2 n_fp64, slots)): evaluations/s if only the FP64 pipe were the limit."""
+    return n_sm * 4 * 32.0 * sm_mhz * 1e6 / (FP64_CLK_PER_WARP_INST * fp64_ops_per_eval(w))
+
+
 def other_roofs(w, n_sm, sm_mhz):
     """The roofs BASELINE.json's metric names, for the integrand's operation mix, next to the IMAD.WIDE roof that binds:
     FP32: 128 lanes per SM per clock; XU (F2F.F64.F32, MUFU): one warp-instruction per 8.5 clocks per scheduler (measured,
     profiles/r1_microbench.md) = 15.06 lanes per SM per clock."""
     f = sm_mhz * 1e6
+    if w.precision == "f64":
+        return {"imad_wide_gevals_per_s": alu_peak_evals_per_s(w.dim, n_sm, sm_mhz) / 1e9,
+                "fp64_pipe_gevals_per_s": fp64_peak_evals_per_s(w, n_sm, sm_mhz) / 1e9,
+                "note": "evaluations/s if only that pipe were the limit (FP64 mode: %d FP64 instructions at %g clocks and %g IMAD.WIDE at 4 clocks per "
+                        "warp-evaluation; the roof is the lower of the two)" % (fp64_ops_per_eval(w), FP64_CLK_PER_WARP_INST, PHILOX_IMAD_WIDE_PER_CALL * calls_per_eval(w.dim))}
     return {"fp32_fma_gevals_per_s": n_sm * 128.0 * f / fp32_ops_per_eval(w) / 1e9,
             "xu_gevals_per_s": n_sm * 4 * 32.0 / 8.5 * f / 1.0 / 1e9,
             "note": "evaluations/s if only that pipe were the limit (exact mode: %d FP32 instructions and 1 XU conversion per evaluation)" % fp32_ops_per_eval(w)}
@@ -379,6 +405,8 @@ def main():
         pass
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = alu_peak_evals_per_s(w.dim, n_sm, sm_max)
+    if w.precision == "f64":      # C = max(4 n_imad, 2 n_fp64): whichever pipe is the slower one
+        peak = min(peak, fp64_peak_evals_per_s(w, n_sm, sm_max))
     traffic, traffic_commit = traffic_from_profiles(args.workload, args.math)
     peak_issued = n_sm * sm_max * 1e6 * 32.0 / (IMAD_WIDE_CLK_PER_WARP_INST_PER_SM * imad_wide_issued_per_eval(w.dim))
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s", "frac": achieved / peak,

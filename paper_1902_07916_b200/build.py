@@ -8,9 +8,6 @@ Steps
   2. nvcc -c, in parallel: zmc_lib.cu, zmc_static.cu and zmc_inst.cu once per pre-compiled
      (precision, math mode, integrand) combination;
   3. nvcc -shared -cudart static -> paper_1902_07916_b200/libzmc.so.
-build_microbench() makes the pipe-rate probes of csrc/zmc_microbench.cu a library of their own
-(libzmc_microbench.so, used by `python -m paper_1902_07916_b200.microbench` only): they are not part of the product ABI.
-
 Flags: -gencode arch=compute_100a,code=sm_100a (B200 only), -lineinfo (ncu source pages),
 --fmad=false (every fused multiply-add in the device code is written explicitly; R8).
 nvcc cross-compiles without a GPU, so this runs in the CPU-only build container too.
@@ -72,7 +69,7 @@ def _sources():
 def _stamp() -> str:
     h = hashlib.sha256()
     for name in sorted(os.listdir(CSRC)):
-        if name.endswith((".cu", ".cuh", ".h")) and name not in ("zmc_microbench.cu", "zmc_kernel_probe.cu"):
+        if name.endswith((".cu", ".cuh", ".h")):
             h.update(name.encode())
             h.update(open(os.path.join(CSRC, name), "rb").read())
     h.update(open(os.path.join(os.path.dirname(HERE), "include", "zmc.h"), "rb").read())
@@ -121,22 +118,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with open(stamp_file, "w") as f:
         f.write(stamp)
     return LIB
-
-
-MICROBENCH_LIB = os.path.join(HERE, "libzmc_microbench.so")
-
-
-def build_microbench(force: bool = False) -> str:
-    """The issue-rate probes (profiles/r1_microbench.md) as their own small library; not linked into libzmc.so."""
-    src = os.path.join(CSRC, "zmc_microbench.cu")
-    deps = [src, os.path.join(CSRC, "zmc_device.cuh")]
-    if not force and os.path.exists(MICROBENCH_LIB) and all(os.path.getmtime(MICROBENCH_LIB) >= os.path.getmtime(d) for d in deps):
-        return MICROBENCH_LIB
-    cmd = [NVCC, *NVCC_FLAGS, "-shared", "-cudart", "static", "-o", MICROBENCH_LIB, src]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError("nvcc failed for zmc_microbench:\n%s\n%s" % (" ".join(cmd), r.stderr[-6000:]))
-    return MICROBENCH_LIB
 
 
 if __name__ == "__main__":

@@ -326,6 +326,37 @@ struct ZmcMapF32 {
     }
 };
 
+/* ------------------------------------------------------------------ FP64 sine (R8: FP64 values within 4 ulp of the CPU's libm) */
+/* The FP32 scheme at FP64 length, branch-free: k = rint(a/pi) by the magic-number add, three-constant Cody-Waite reduction with FMAs
+ * (a - k*PI_HI is exact: a multiple of 2^-51 below 1.6), odd polynomial of degree 17 on [-pi/2, pi/2] (near-minimax: interpolation of
+ * (sin(r)/r - 1)/r^2 at 8 Chebyshev nodes in r^2), sign (-1)^k from the low bit of the magic sum. 15 FP64 instructions against ~28 of
+ * libdevice's sin with its quadrant selection, and no call. Measured against sinl on the host with the same operations (gcc, fma()):
+ * at most 1.94 ulp for |a| <= 1e9 (the worst cases sit at |r| near pi/2, where r + r^3 p cancels 1.57 - 0.57), 0.99 ulp at a = fl(k pi);
+ * libm itself is within 0.52, so the two sides differ by at most 2.5 ulp. Beyond 2^30 (k*PI_LO's own error starts to show in r):
+ * libdevice's sin, with its Payne-Hanek reduction. */
+static __device__ __noinline__ double zmc_sin_far(double a) { return sin(a); }      /* one cold copy per program, called: not inlined into every sample loop */
+
+__device__ __forceinline__ double zmc_zsin64(double a) {
+    if (!(fabs(a) <= 1073741824.0)) return zmc_sin_far(a);      /* also NaN and infinity */
+    const double MAGIC = 6755399441055744.0;            /* 1.5 * 2^52: adding it rounds to an integer in the low mantissa bits */
+    const double t = __fma_rn(a, __longlong_as_double(0x3fd45f306dc9c883ll), MAGIC);       /* a/pi + MAGIC */
+    const double kd = __dadd_rn(t, -MAGIC);
+    double r = __fma_rn(-kd, __longlong_as_double(0x400921fb54442d18ll), a);                /* PI_HI */
+    r = __fma_rn(-kd, __longlong_as_double(0x3ca1a62633145c07ll), r);                        /* PI_MID */
+    r = __fma_rn(-kd, __longlong_as_double(0xb92f1976b7ed8fbcll), r);                        /* PI_LO */
+    const double r2 = __dmul_rn(r, r);
+    double p = __longlong_as_double(0x3ce892efd890db97ll);                                   /* r^17 */
+    p = __fma_rn(p, r2, __longlong_as_double(0xbd6ae4d771729416ll));
+    p = __fma_rn(p, r2, __longlong_as_double(0x3de6123f55a16315ll));
+    p = __fma_rn(p, r2, __longlong_as_double(0xbe5ae64557c0cbf9ll));
+    p = __fma_rn(p, r2, __longlong_as_double(0x3ec71de3a5419df5ll));
+    p = __fma_rn(p, r2, __longlong_as_double(0xbf2a01a01a0184f4ll));
+    p = __fma_rn(p, r2, __longlong_as_double(0x3f81111111111104ll));
+    p = __fma_rn(p, r2, __longlong_as_double(0xbfc5555555555555ll));                         /* r^3 */
+    const double v = __fma_rn(__dmul_rn(r, r2), p, r);
+    return __hiloint2double(__double2hiint(v) ^ (__double2loint(t) << 31), __double2loint(v));
+}
+
 template <int D>
 struct ZmcMapF64 {
     double lo[D], step[D];
@@ -589,7 +620,7 @@ struct ZmcIntegrand<ID, D_, ZMC_PREC_F64, MODE> {
             double s = x[0];
 #pragma unroll
             for (int d = 1; d < D_; ++d) s = __dadd_rn(s, x[d]);
-            return sin(s);
+            return zmc_zsin64(s);
         }
         if (ID == ZMC_ID_EXP_QUAD) {
             double q = 0.0;
@@ -713,31 +744,15 @@ __host__ __device__ constexpr bool zmc_tune_trial_loop(int D) { return D != 6; }
 template <class F>
 struct ZmcTune {
     static constexpr int D = F::D;
-#ifdef ZMC_TUNE_PACKED      /* tuning sweeps override all three from the command line */
-    static constexpr bool PACKED = F::HAS_PACKED && (ZMC_TUNE_PACKED != 0);
-    static constexpr int UNROLL = ZMC_TUNE_UNROLL;
-    static constexpr int MINB = ZMC_TUNE_MINB;
-#ifdef ZMC_TUNE_P0ADD
-    static constexpr bool P0_ADD = (ZMC_TUNE_P0ADD != 0);
-    static constexpr bool P0_CARRY = (ZMC_TUNE_P0ADD == 2);
-#else
-    static constexpr bool P0_ADD = false;
-    static constexpr bool P0_CARRY = false;
-#endif
-#else
     static constexpr bool PACKED = F::HAS_PACKED;
     static constexpr int UNROLL = (D == 4 || D == 6 || D == 12) ? 4 : 2;
     static constexpr bool P0_ADD = (D == 4 || D == 6 || D == 12);   /* +3.7 % at D = 6, +1 % at D = 4 and 12, -1.5 % at D = 9 */
     static constexpr bool P0_CARRY = P0_ADD;
-    static constexpr int MINB = (F::PREC == ZMC_PREC_F64 && D >= 7) ? 2 : 3;   /* FP64 at high D spills below 255 registers */
-#endif
-#ifdef ZMC_TUNE_ITEM      /* bit 0: FAST_DECODE, bit 1: TRIAL_LOOP */
-    static constexpr bool FAST_DECODE = (ZMC_TUNE_ITEM & 1) != 0;
-    static constexpr bool TRIAL_LOOP = (ZMC_TUNE_ITEM & 2) != 0;
-#else
+    /* FP64: at high D the kernel spills below 255 registers (2 CTAs; the 9-D Gaussian keeps 16 bytes of spill even there); the FP64 6-D kernel is
+     * latency-bound and gains from a fifth CTA per SM (90 registers instead of 104: 0.551 -> 0.567 of the roof, profiles/r3_fp64_pipe_split.md) */
+    static constexpr int MINB = (F::PREC == ZMC_PREC_F64) ? (D >= 7 ? 2 : (D == 6 ? 4 : 3)) : 3;
     static constexpr bool FAST_DECODE = true;
     static constexpr bool TRIAL_LOOP = zmc_tune_trial_loop(D);
-#endif
 };
 
 /* R13: q + f*f. FP32-mode values have 24 significant bits, so the product is exact and one DFMA is the
