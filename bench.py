@@ -413,6 +413,9 @@ def main():
                 "frac_algorithmic": achieved / peak,
                 # the same time against the multiplies the kernel really issues (FP32 built-ins): the share of the time the FMA-heavy pipe spends on them
                 "frac_pipe": (achieved / peak_issued) if w.precision == "f32" else None,
+                # FP64 mode, measured (profiles/r3_fp64_pipe_split.md): on B200 the FP64 pipe and the FMA-heavy pipe do not overlap -- their busy cycles ADD UP to the
+                # elapsed ones -- so the time that cannot be undercut is 4 n_imad + 2 n_fp64 clocks per warp-evaluation, not the larger of the two
+                "frac_shared_pipe": (achieved / (1.0 / (1.0 / alu_peak_evals_per_s(w.dim, n_sm, sm_max) + 1.0 / fp64_peak_evals_per_s(w, n_sm, sm_max)))) if w.precision == "f64" else None,
                 "imad_wide_per_eval": {"algorithmic": PHILOX_IMAD_WIDE_PER_CALL * calls_per_eval(w.dim), "issued": imad_wide_issued_per_eval(w.dim)},
                 "other_roofs": other_roofs(w, n_sm, sm_max),
                 "traffic": traffic,
